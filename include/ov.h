@@ -1,0 +1,142 @@
+/*
+ * ov.h -- C ABI of the B200-native overlap-operator library (libov.so).
+ *
+ * The hot path of arXiv 1111.6288: applying D_ov = 1 + gamma5 sign(H_w), H_w = gamma5 D_w
+ * (eq. 2.1), with sign(H_w) ~ Q P(Q^2), Q = H_w/||H_w|| on the "large space"
+ * and the exact sign on the lowest eigenvectors of Q, the "small space".
+ * Consumers/producers on the same kernels: a multi-mass CG and an eigensolver for the
+ * low modes of H_w.  Readings of points the paper leaves open: DESIGN.md.
+ *
+ * Conventions
+ *   - every call returns an int status: OV_OK or an OV_E* code; nothing throws or aborts across the ABI;
+ *     ov_last_error(ctx) gives a NUL-terminated message owned by ctx (valid until the next call).
+ *   - "dev" pointers are CUDA device pointers (fp64); "host" pointers are ordinary host memory.
+ *   - all device work is enqueued on the cudaStream_t given to ov_create; calls that return host
+ *     scalars (dot/norm, CG, Lanczos, *_host variants) synchronise that stream before returning.
+ *   - in/out aliasing is forbidden for every apply call (the operator is a stencil) -> OV_EINVAL.
+ *   - there is no CPU fallback: without a usable CUDA device every compute call returns OV_ECUDA.
+ *
+ * Lattice: dims = {X,Y,Z,T}; site index i = x + X*(y + Y*(z + Z*t)); V = X*Y*Z*T sites; directions
+ * mu = 0..3 = x,y,z,t; periodic in x,y,z, antiperiodic in t (the hop between t=T-1 and t=0 carries -1).
+ * gamma matrices: Hermitian chiral basis, gamma5 = diag(1,1,-1,-1) (reading G2).
+ *
+ * Layouts
+ *   canonical gauge   complex128 [T][Z][Y][X][mu][row][col]   U_mu(x) links x -> x+mu
+ *   canonical spinor  complex128 [T][Z][Y][X][spin][colour]   (= [site][12])
+ *   ABI spinor ("SoA") complex128 [12][V]: component (spin s, colour c) of site i at complex index
+ *                     (3*s+c)*V + i, (re,im) interleaved.  nrhs vectors are consecutive (stride 12*V).
+ *                     ov_pack_spinor / ov_unpack_spinor convert canonical <-> ABI on the device.
+ */
+#ifndef OV_H_
+#define OV_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    OV_OK = 0,
+    OV_EINVAL = 1,  /* bad argument (null, aliasing, bad dims, lambda == 0, ...)          */
+    OV_ENOMEM = 2,  /* device allocation failed                                            */
+    OV_ECUDA = 3,   /* CUDA runtime/driver error (message has the CUDA error string)       */
+    OV_ESTATE = 4,  /* call order: e.g. ov_apply_sign before ov_set_polynomial             */
+    OV_ENOCONV = 5  /* iterative routine hit its iteration limit; outputs hold the last iterate */
+};
+
+typedef struct ov_ctx ov_ctx;
+
+/* ---- lifetime ------------------------------------------------------------------------------------
+ * ov_create: builds a context for one gauge field.  gauge_dev: canonical gauge on the DEVICE; it is
+ * COPIED and re-laid out (site-major SoA, row-major 3x3 per link; recon = 18 keeps all 9 complex
+ * entries, recon = 12 keeps rows 0-1 and rebuilds row 2 = conj(row0 x row1) in registers, valid for
+ * SU(3) links only).  The caller may free gauge_dev after the call returns (the call synchronises).
+ * kappa = 1/(2(m0+4)) is the Wilson hopping parameter (reading G1).
+ * cuda_stream: a cudaStream_t (NULL = legacy default stream).                                        */
+int ov_create(ov_ctx** out, const int dims[4], double kappa, const void* gauge_dev, int recon,
+              void* cuda_stream);
+void ov_destroy(ov_ctx* ctx);
+const char* ov_last_error(const ov_ctx* ctx);
+size_t ov_spinor_bytes(const ov_ctx* ctx); /* 192 * V */
+long long ov_volume(const ov_ctx* ctx);
+/* number of CUDA kernels this context has launched since creation (for bench.py's gpu_launches) */
+long long ov_launch_count(const ov_ctx* ctx);
+/* selects the dslash kernel: 0 = automatic, 1 = gather (one thread per site, cache-reliant),
+ * 2 = tiled (shared-memory staged).  Returns OV_EINVAL if the variant cannot run on this lattice. */
+int ov_set_dslash_variant(ov_ctx* ctx, int variant);
+
+/* ---- layout ------------------------------------------------------------------- */
+int ov_pack_spinor(ov_ctx* ctx, const void* canonical_dev, void* abi_dev, int nrhs);
+int ov_unpack_spinor(ov_ctx* ctx, const void* abi_dev, void* canonical_dev, int nrhs);
+
+/* ---- Wilson kernel (row a2) -----------------------------------------------------
+ * ov_dslash:   out = sum_mu [ s+ (1-gamma_mu) U_mu(x) in(x+mu) + s- (1+gamma_mu) U_mu(x-mu)^+ in(x-mu) ]
+ * ov_apply_hw: out = H_w in = gamma5 (in - kappa * dslash(in))      (NOT divided by the norm)
+ * in/out: ABI spinors on the device, nrhs of them.                                                   */
+int ov_dslash(ov_ctx* ctx, const void* in, void* out, int nrhs);
+int ov_apply_hw(ov_ctx* ctx, const void* in, void* out, int nrhs);
+
+/* ---- polynomial (row a3; eq. 2.2) ----------------------------------------------------
+ * ov_chebyshev_coeffs: host helper.  Fills coeffs_host[0..order] with the Chebyshev-interpolation
+ *   coefficients of x^(-1/2) on [eps,1] in the basis T_j(z), z = (2x-1-eps)/(1-eps); coeffs[0] is the
+ *   true T_0 coefficient (P = sum_j c_j T_j, no 1/2 applied anywhere else).
+ * ov_set_polynomial: coeffs are COPIED.  order = degree n of P in x = Q^2 (2n+1 H_w applications per
+ *   sign).  norm >= ||H_w|| defines Q = H_w/norm; eps > 0: P approximates x^(-1/2) on [eps,1].        */
+int ov_chebyshev_coeffs(int order, double eps, double* coeffs_host);
+int ov_set_polynomial(ov_ctx* ctx, const double* coeffs_host, int order, double eps, double norm);
+
+/* ---- small space (row a4) -------------------------------------------------------
+ * V_dev: k orthonormal ABI spinors, contiguous, on the device: BORROWED, never copied (it is 17-80 GB
+ * at the paper's sizes); the caller keeps it alive until it is replaced, k = 0 is set, or the context
+ * is destroyed.  lambda_host: the k eigenvalues of Q = H_w/norm (for the norm last set), COPIED;
+ * lambda == 0 is rejected (OV_EINVAL).  k = 0 disables the small space.                              */
+int ov_set_smallspace(ov_ctx* ctx, const void* V_dev, const double* lambda_host, int k);
+/* test/bench hook for the projector alone: c = V^+ in (k complex, to coef_host if non-NULL),
+ * perp = in - V c,  low = V (sign(lambda) o c).  perp/low: ABI spinors on the device.                 */
+int ov_project(ov_ctx* ctx, const void* in, void* perp, void* low, double* coef_host);
+
+/* ---- the operator (rows a3-a5) ----------------------------------------------------
+ * ov_apply_sign: out = sum_i sign(lambda_i) v_i (v_i^+ in) + Q P(Q^2) (1 - V V^+) in
+ * ov_apply_dov:  out = (1 + mass/2) in + (1 - mass/2) gamma5 sign(H_w) in     (mass = 0: eq. 2.1)
+ * The *_host variants take canonical HOST spinors, copy them to the device, run the same device path
+ * and copy the canonical result back (synchronous) -- the end-to-end entry point bench.py times.     */
+int ov_apply_sign(ov_ctx* ctx, const void* in, void* out, int nrhs);
+int ov_apply_dov(ov_ctx* ctx, double mass, const void* in, void* out, int nrhs);
+int ov_apply_hw_host(ov_ctx* ctx, const void* in_host, void* out_host, int nrhs);
+int ov_apply_dov_host(ov_ctx* ctx, double mass, const void* in_host, void* out_host, int nrhs);
+
+/* ---- BLAS-1 hooks (row a6; "vector additions and scalar products") --------------------
+ * Vectors are ABI spinors on the device.  Reductions are two-stage with a fixed shape (no atomics), so
+ * results are bit-reproducible from run to run.  dot = sum conj(x) y -> out_host[2] = (re, im).       */
+int ov_blas_axpy(ov_ctx* ctx, double a_re, double a_im, const void* x, void* y); /* y += a x */
+int ov_blas_scale(ov_ctx* ctx, double a, void* x);
+int ov_blas_dot(ov_ctx* ctx, const void* x, const void* y, double* out_host);
+int ov_blas_norm2(ov_ctx* ctx, const void* x, double* out_host);
+
+/* ---- consumers -------------------------------------------------------------------------------------
+ * ov_multishift_cg (row a7): solves (A + sigma_i) x_i = b, A = D_ov(0)^+ D_ov(0) applied as
+ *   gamma5 D_ov gamma5 D_ov, sigma_i = m_i^2/(1 - m_i^2/4) (reading G10).  b: one ABI spinor; x: nmass
+ *   ABI spinors (overwritten, initial guess 0).  Stops when the slowest system has |r| <= tol |b|.
+ *   iters_out: iterations; relres_out[nmass]: TRUE relative residuals recomputed with A at the end.
+ *   Returns OV_ENOCONV if maxiter was hit.
+ * ov_lanczos_lowmodes (row a8): the k eigenpairs of Q = H_w/norm of smallest |lambda|,
+ *   by Chebyshev-filtered thick-restart Lanczos on Q^2 followed by Rayleigh-Ritz in Q.  Needs the norm
+ *   from ov_set_polynomial.  V_out_dev: k ABI spinors; lambda_out_host, resid_out_host: k values,
+ *   resid_i = |Q v_i - lambda_i v_i|.  Returns OV_ENOCONV if some resid_i > tol after max_restarts.
+ *   subspace = Krylov dimension m (0 = default 2k+16; the paper uses 2.5 k); cheb_order = degree of the
+ *   filter in Q^2 (paper: 100).                                                                        */
+int ov_multishift_cg(ov_ctx* ctx, const double* masses_host, int nmass, const void* b, void* x, double tol,
+                     int maxiter, int* iters_out, double* relres_out);
+int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_restarts, int cheb_order, int subspace,
+                        void* V_out_dev, double* lambda_out_host, double* resid_out_host);
+
+/* ---- host-logic test hook (no device work): eigen-decomposition of a dense n x n Hermitian matrix by the
+ * cyclic complex Jacobi routine the Lanczos driver uses.  A_host: row-major (re,im) pairs; w_out: n ascending
+ * eigenvalues; Z_out: row-major (re,im), eigenvectors as columns.                                            */
+int ov_host_eigh(int n, const double* A_host, double* w_out, double* Z_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* OV_H_ */

@@ -1,0 +1,168 @@
+// C ABI entry points (include/ov.h): argument checks, context lifetime, workspaces.
+#include <cmath>
+#include <cstring>
+
+#include "ov_internal.h"
+
+namespace ov {
+
+int fail(const ov_ctx* ctx, int code, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (ctx) ctx->err = buf;
+    return code;
+}
+
+int cuda_fail(const ov_ctx* ctx, cudaError_t e, const char* what) {
+    return fail(ctx, e == cudaErrorMemoryAllocation ? OV_ENOMEM : OV_ECUDA, "CUDA error '%s' in %s",
+                cudaGetErrorString(e), what);
+}
+
+int workspace(ov_ctx* ctx, int i, double2** out) {
+    if (!ctx->ws[i]) OV_CUDA(ctx, cudaMalloc(&ctx->ws[i], spinor_elems(ctx) * sizeof(double2)));
+    *out = ctx->ws[i];
+    return OV_OK;
+}
+
+int ensure_reduction_buffers(ov_ctx* ctx, size_t partial_elems, size_t result_elems) {
+    if (partial_elems > ctx->partial_cap) {
+        OV_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        if (ctx->d_partial) cudaFree(ctx->d_partial);
+        ctx->d_partial = nullptr;
+        ctx->partial_cap = 0;
+        OV_CUDA(ctx, cudaMalloc(&ctx->d_partial, partial_elems * sizeof(double2)));
+        ctx->partial_cap = partial_elems;
+    }
+    if (result_elems > ctx->result_cap) {
+        OV_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        if (ctx->d_result) cudaFree(ctx->d_result);
+        if (ctx->h_result) cudaFreeHost(ctx->h_result);
+        ctx->d_result = nullptr;
+        ctx->h_result = nullptr;
+        ctx->result_cap = 0;
+        const size_t cap = result_elems < 1024 ? 1024 : result_elems;
+        OV_CUDA(ctx, cudaMalloc(&ctx->d_result, cap * sizeof(double2)));
+        OV_CUDA(ctx, cudaMallocHost(&ctx->h_result, cap * sizeof(double2)));
+        ctx->result_cap = cap;
+    }
+    return OV_OK;
+}
+
+int launch_wilson(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep) {
+    const int v = ctx->dslash_variant;
+    if (v == 2 || (v == 0 && tiled_supported(ctx))) return launch_wilson_tiled(ctx, in, out, ep);
+    return launch_wilson_gather(ctx, in, out, ep);
+}
+
+static bool overlaps(const ov_ctx* ctx, const void* a, const void* b, int nrhs) {
+    const char* pa = (const char*)a;
+    const char* pb = (const char*)b;
+    const size_t n = spinor_elems(ctx) * sizeof(double2) * (size_t)nrhs;
+    return pa < pb + n && pb < pa + n;
+}
+
+static int check_apply(ov_ctx* ctx, const void* in, void* out, int nrhs) {
+    if (!ctx) return OV_EINVAL;
+    if (!in || !out || nrhs < 1) return fail(ctx, OV_EINVAL, "null pointer or nrhs < 1");
+    if (overlaps(ctx, in, out, nrhs)) return fail(ctx, OV_EINVAL, "in and out overlap (the operator is a stencil)");
+    return OV_OK;
+}
+
+}  // namespace ov
+
+using namespace ov;
+
+extern "C" {
+
+int ov_create(ov_ctx** out, const int dims[4], double kappa, const void* gauge_dev, int recon, void* cuda_stream) {
+    if (!out) return OV_EINVAL;
+    *out = nullptr;
+    if (!dims || !gauge_dev) return OV_EINVAL;
+    if (recon != 18 && recon != 12) return OV_EINVAL;
+    for (int d = 0; d < 4; d++)
+        if (dims[d] < 2) return OV_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return OV_ECUDA;  // no CPU fallback
+    ov_ctx* ctx = new ov_ctx();
+    ctx->lat.X = dims[0]; ctx->lat.Y = dims[1]; ctx->lat.Z = dims[2]; ctx->lat.T = dims[3];
+    ctx->lat.V = (long long)dims[0] * dims[1] * dims[2] * dims[3];
+    ctx->kappa = kappa;
+    ctx->recon = recon;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    const size_t gbytes = (size_t)4 * (recon / 2) * ctx->lat.V * sizeof(double2);
+    cudaError_t e = cudaMalloc(&ctx->gauge, gbytes);
+    if (e != cudaSuccess) { delete ctx; return e == cudaErrorMemoryAllocation ? OV_ENOMEM : OV_ECUDA; }
+    int rc = launch_gauge_relayout(ctx, (const double2*)gauge_dev);
+    if (rc == OV_OK && cudaStreamSynchronize(ctx->stream) != cudaSuccess) rc = OV_ECUDA;
+    if (rc == OV_OK) rc = ensure_reduction_buffers(ctx, 1, 1024);
+    if (rc != OV_OK) { ov_destroy(ctx); return rc; }
+    *out = ctx;
+    return OV_OK;
+}
+
+void ov_destroy(ov_ctx* ctx) {
+    if (!ctx) return;
+    cudaStreamSynchronize(ctx->stream);
+    cudaFree(ctx->gauge);
+    for (auto& w : ctx->ws) cudaFree(w);
+    cudaFree(ctx->d_partial);
+    cudaFree(ctx->d_result);
+    if (ctx->h_result) cudaFreeHost(ctx->h_result);
+    cudaFree(ctx->d_sgn);
+    cudaFree(ctx->d_coef);
+    cudaFree(ctx->host_stage_in);
+    cudaFree(ctx->host_stage_abi);
+    cudaFree(ctx->host_stage_out);
+    delete ctx;
+}
+
+const char* ov_last_error(const ov_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+size_t ov_spinor_bytes(const ov_ctx* ctx) { return ctx ? spinor_elems(ctx) * sizeof(double2) : 0; }
+long long ov_volume(const ov_ctx* ctx) { return ctx ? ctx->lat.V : 0; }
+long long ov_launch_count(const ov_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int ov_set_dslash_variant(ov_ctx* ctx, int variant) {
+    if (!ctx) return OV_EINVAL;
+    if (variant < 0 || variant > 2) return fail(ctx, OV_EINVAL, "variant must be 0, 1 or 2");
+    if (variant == 2 && !tiled_supported(ctx)) return fail(ctx, OV_EINVAL, "tiled dslash does not support this lattice");
+    ctx->dslash_variant = variant;
+    return OV_OK;
+}
+
+int ov_pack_spinor(ov_ctx* ctx, const void* canonical_dev, void* abi_dev, int nrhs) {
+    OV_TRY(check_apply(ctx, canonical_dev, abi_dev, nrhs));
+    const size_t n = spinor_elems(ctx);
+    for (int r = 0; r < nrhs; r++)
+        OV_TRY(launch_pack(ctx, (const double2*)canonical_dev + r * n, (double2*)abi_dev + r * n));
+    return OV_OK;
+}
+
+int ov_unpack_spinor(ov_ctx* ctx, const void* abi_dev, void* canonical_dev, int nrhs) {
+    OV_TRY(check_apply(ctx, abi_dev, canonical_dev, nrhs));
+    const size_t n = spinor_elems(ctx);
+    for (int r = 0; r < nrhs; r++)
+        OV_TRY(launch_unpack(ctx, (const double2*)abi_dev + r * n, (double2*)canonical_dev + r * n));
+    return OV_OK;
+}
+
+int ov_dslash(ov_ctx* ctx, const void* in, void* out, int nrhs) {
+    OV_TRY(check_apply(ctx, in, out, nrhs));
+    const size_t n = spinor_elems(ctx);
+    Epilogue ep;
+    ep.hop_only = 1;
+    for (int r = 0; r < nrhs; r++) OV_TRY(launch_wilson(ctx, (const double2*)in + r * n, (double2*)out + r * n, ep));
+    return OV_OK;
+}
+
+int ov_apply_hw(ov_ctx* ctx, const void* in, void* out, int nrhs) {
+    OV_TRY(check_apply(ctx, in, out, nrhs));
+    const size_t n = spinor_elems(ctx);
+    Epilogue ep;  // s = 1, gamma5
+    for (int r = 0; r < nrhs; r++) OV_TRY(launch_wilson(ctx, (const double2*)in + r * n, (double2*)out + r * n, ep));
+    return OV_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,169 @@
+// C ABI entry points, part 2: polynomial, small space, sign / D_ov, host-buffer variants, BLAS hooks.
+#include <cmath>
+#include <cstring>
+
+#include "ov_internal.h"
+
+using namespace ov;
+
+static bool overlaps2(const ov_ctx* ctx, const void* a, const void* b, int nrhs) {
+    const char* pa = (const char*)a;
+    const char* pb = (const char*)b;
+    const size_t n = spinor_elems(ctx) * sizeof(double2) * (size_t)nrhs;
+    return pa < pb + n && pb < pa + n;
+}
+static int check2(ov_ctx* ctx, const void* in, void* out, int nrhs) {
+    if (!ctx) return OV_EINVAL;
+    if (!in || !out || nrhs < 1) return fail(ctx, OV_EINVAL, "null pointer or nrhs < 1");
+    if (overlaps2(ctx, in, out, nrhs)) return fail(ctx, OV_EINVAL, "in and out overlap (the operator is a stencil)");
+    return OV_OK;
+}
+
+extern "C" {
+
+// Chebyshev interpolation of x^(-1/2) on [eps,1] at the order+1 first-kind nodes (O5, reading G4/G5).
+int ov_chebyshev_coeffs(int order, double eps, double* coeffs_host) {
+    if (order < 0 || !(eps > 0.0) || !(eps < 1.0) || !coeffs_host) return OV_EINVAL;
+    const int m = order + 1;
+    const long double pi = 3.141592653589793238462643383279502884L;
+    std::vector<long double> f(m), th(m);
+    for (int k = 0; k < m; k++) {
+        th[k] = pi * (k + 0.5L) / m;
+        const long double x = 0.5L * ((1.0L - eps) * cosl(th[k]) + 1.0L + eps);
+        f[k] = 1.0L / sqrtl(x);
+    }
+    for (int j = 0; j < m; j++) {
+        long double s = 0.0L;
+        for (int k = 0; k < m; k++) s += f[k] * cosl(j * th[k]);
+        s *= 2.0L / m;
+        if (j == 0) s *= 0.5L;
+        coeffs_host[j] = (double)s;
+    }
+    return OV_OK;
+}
+
+int ov_set_polynomial(ov_ctx* ctx, const double* coeffs_host, int order, double eps, double norm) {
+    if (!ctx) return OV_EINVAL;
+    if (!coeffs_host || order < 0) return fail(ctx, OV_EINVAL, "null coefficients or negative order");
+    if (!(eps > 0.0) || !(eps < 1.0)) return fail(ctx, OV_EINVAL, "eps must lie in (0,1)");
+    if (!(norm > 0.0)) return fail(ctx, OV_EINVAL, "norm must be positive");
+    for (int j = 0; j <= order; j++)
+        if (!std::isfinite(coeffs_host[j])) return fail(ctx, OV_EINVAL, "coefficient %d is not finite", j);
+    ctx->coef.assign(coeffs_host, coeffs_host + order + 1);
+    ctx->order = order;
+    ctx->eps = eps;
+    ctx->norm = norm;
+    return OV_OK;
+}
+
+int ov_set_smallspace(ov_ctx* ctx, const void* V_dev, const double* lambda_host, int k) {
+    if (!ctx) return OV_EINVAL;
+    if (k < 0) return fail(ctx, OV_EINVAL, "k < 0");
+    if (k == 0) { ctx->k = 0; ctx->Vlow = nullptr; ctx->lambda.clear(); return OV_OK; }
+    if (!V_dev || !lambda_host) return fail(ctx, OV_EINVAL, "null V or lambda with k > 0");
+    if ((size_t)k * 2 * sizeof(double2) > 200 * 1024) return fail(ctx, OV_EINVAL, "k too large (max 6400)");
+    std::vector<double> sgn(k);
+    for (int i = 0; i < k; i++) {
+        if (lambda_host[i] == 0.0 || !std::isfinite(lambda_host[i]))
+            return fail(ctx, OV_EINVAL, "lambda[%d] is zero or not finite: sign undefined (reading G8)", i);
+        sgn[i] = lambda_host[i] > 0 ? 1.0 : -1.0;
+    }
+    if (k > ctx->cap_k) {
+        OV_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        cudaFree(ctx->d_sgn); cudaFree(ctx->d_coef);
+        ctx->d_sgn = nullptr; ctx->d_coef = nullptr; ctx->cap_k = 0;
+        OV_CUDA(ctx, cudaMalloc(&ctx->d_sgn, (size_t)k * sizeof(double)));
+        OV_CUDA(ctx, cudaMalloc(&ctx->d_coef, (size_t)k * 2 * sizeof(double2)));
+        ctx->cap_k = k;
+    }
+    OV_CUDA(ctx, cudaMemcpyAsync(ctx->d_sgn, sgn.data(), (size_t)k * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    OV_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    ctx->Vlow = (const double2*)V_dev;
+    ctx->lambda.assign(lambda_host, lambda_host + k);
+    ctx->k = k;
+    return OV_OK;
+}
+
+int ov_project(ov_ctx* ctx, const void* in, void* perp, void* low, double* coef_host) {
+    if (!ctx) return OV_EINVAL;
+    if (!in || !perp || !low) return fail(ctx, OV_EINVAL, "null pointer");
+    if (ctx->k <= 0) return fail(ctx, OV_ESTATE, "no small space set");
+    OV_TRY(project(ctx, (const double2*)in, (double2*)perp, (double2*)low));
+    if (coef_host) {
+        std::vector<double2> c(ctx->k);
+        OV_TRY(fetch_results(ctx, ctx->k, c.data()));
+        for (int i = 0; i < ctx->k; i++) { coef_host[2 * i] = c[i].x; coef_host[2 * i + 1] = c[i].y; }
+    }
+    return OV_OK;
+}
+
+int ov_apply_sign(ov_ctx* ctx, const void* in, void* out, int nrhs) {
+    OV_TRY(check2(ctx, in, out, nrhs));
+    const size_t n = spinor_elems(ctx);
+    for (int r = 0; r < nrhs; r++) OV_TRY(apply_sign(ctx, (const double2*)in + r * n, (double2*)out + r * n));
+    return OV_OK;
+}
+
+int ov_apply_dov(ov_ctx* ctx, double mass, const void* in, void* out, int nrhs) {
+    OV_TRY(check2(ctx, in, out, nrhs));
+    const size_t n = spinor_elems(ctx);
+    for (int r = 0; r < nrhs; r++) OV_TRY(apply_dov(ctx, mass, (const double2*)in + r * n, (double2*)out + r * n));
+    return OV_OK;
+}
+
+// host-buffer path: H2D -> pack -> operator -> unpack -> D2H, one RHS at a time through 3 device stages
+static int host_apply(ov_ctx* ctx, int which, double mass, const void* in_host, void* out_host, int nrhs) {
+    if (!ctx) return OV_EINVAL;
+    if (!in_host || !out_host || nrhs < 1) return fail(ctx, OV_EINVAL, "null pointer or nrhs < 1");
+    const size_t n = spinor_elems(ctx), bytes = n * sizeof(double2);
+    if (!ctx->host_stage_in) OV_CUDA(ctx, cudaMalloc(&ctx->host_stage_in, bytes));
+    if (!ctx->host_stage_abi) OV_CUDA(ctx, cudaMalloc(&ctx->host_stage_abi, bytes));
+    if (!ctx->host_stage_out) OV_CUDA(ctx, cudaMalloc(&ctx->host_stage_out, bytes));
+    for (int r = 0; r < nrhs; r++) {
+        OV_CUDA(ctx, cudaMemcpyAsync(ctx->host_stage_in, (const char*)in_host + r * bytes, bytes, cudaMemcpyHostToDevice, ctx->stream));
+        OV_TRY(launch_pack(ctx, ctx->host_stage_in, ctx->host_stage_abi));
+        if (which == 0) {
+            Epilogue ep;
+            OV_TRY(launch_wilson(ctx, ctx->host_stage_abi, ctx->host_stage_out, ep));
+        } else {
+            OV_TRY(apply_dov(ctx, mass, ctx->host_stage_abi, ctx->host_stage_out));
+        }
+        OV_TRY(launch_unpack(ctx, ctx->host_stage_out, ctx->host_stage_in));
+        OV_CUDA(ctx, cudaMemcpyAsync((char*)out_host + r * bytes, ctx->host_stage_in, bytes, cudaMemcpyDeviceToHost, ctx->stream));
+    }
+    OV_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return OV_OK;
+}
+
+int ov_apply_hw_host(ov_ctx* ctx, const void* in_host, void* out_host, int nrhs) {
+    return host_apply(ctx, 0, 0.0, in_host, out_host, nrhs);
+}
+int ov_apply_dov_host(ov_ctx* ctx, double mass, const void* in_host, void* out_host, int nrhs) {
+    return host_apply(ctx, 1, mass, in_host, out_host, nrhs);
+}
+
+int ov_blas_axpy(ov_ctx* ctx, double a_re, double a_im, const void* x, void* y) {
+    if (!ctx) return OV_EINVAL;
+    if (!x || !y) return fail(ctx, OV_EINVAL, "null pointer");
+    return launch_axpy(ctx, make_double2(a_re, a_im), (const double2*)x, (double2*)y);
+}
+int ov_blas_scale(ov_ctx* ctx, double a, void* x) {
+    if (!ctx) return OV_EINVAL;
+    if (!x) return fail(ctx, OV_EINVAL, "null pointer");
+    return launch_scale(ctx, a, (double2*)x);
+}
+int ov_blas_dot(ov_ctx* ctx, const void* x, const void* y, double* out_host) {
+    if (!ctx) return OV_EINVAL;
+    if (!x || !y || !out_host) return fail(ctx, OV_EINVAL, "null pointer");
+    double2 r;
+    OV_TRY(dot_host(ctx, (const double2*)x, (const double2*)y, &r));
+    out_host[0] = r.x; out_host[1] = r.y;
+    return OV_OK;
+}
+int ov_blas_norm2(ov_ctx* ctx, const void* x, double* out_host) {
+    if (!ctx) return OV_EINVAL;
+    if (!x || !out_host) return fail(ctx, OV_EINVAL, "null pointer");
+    return norm2_host(ctx, (const double2*)x, out_host);
+}
+
+}  // extern "C"

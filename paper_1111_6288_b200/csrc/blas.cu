@@ -1,0 +1,312 @@
+// Layout conversion and BLAS-1 / reduction kernels on ABI spinors (PAPER.md:75
+// "vector additions and scalar products").  Everything here is a pure streaming kernel: the roofline is
+// HBM bandwidth, the design rule is 16-byte coalesced accesses and enough loads in flight per thread.
+// Reductions are two-stage with a fixed shape (warp shuffle -> per-warp partial in global memory ->
+// one block per result summing the partials in a fixed tree), no atomics: bit-reproducible.
+#include "ov_internal.h"
+#include "wilson_math.cuh"
+
+namespace ov {
+
+// ------------------------------------------------------------------------------------------ layout
+// canonical gauge [site][mu][9] -> internal [mu][NE][site]
+template <int NE>
+__global__ void gauge_relayout_kernel(const double2* __restrict__ can, double2* __restrict__ g, long long V) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= V) return;
+#pragma unroll
+    for (int mu = 0; mu < 4; mu++)
+#pragma unroll
+        for (int e = 0; e < NE; e++) g[((long long)mu * NE + e) * V + i] = can[(i * 4 + mu) * 9 + e];
+}
+
+int launch_gauge_relayout(ov_ctx* ctx, const double2* canonical) {
+    const long long V = ctx->lat.V;
+    const int threads = 128;
+    const unsigned blocks = (unsigned)((V + threads - 1) / threads);
+    if (ctx->recon == 12)
+        gauge_relayout_kernel<6><<<blocks, threads, 0, ctx->stream>>>(canonical, ctx->gauge, V);
+    else
+        gauge_relayout_kernel<9><<<blocks, threads, 0, ctx->stream>>>(canonical, ctx->gauge, V);
+    ctx->launches++;
+    OV_CUDA(ctx, cudaGetLastError());
+    return OV_OK;
+}
+
+// canonical spinor [site][12] <-> ABI [12][site], staged through shared memory so both sides coalesce
+constexpr int kPackSites = 128;
+template <bool PACK>
+__global__ void __launch_bounds__(kPackSites) pack_kernel(const double2* __restrict__ src,
+                                                          double2* __restrict__ dst, long long V) {
+    __shared__ double2 tile[kPackSites * 12 + 12];
+    const long long base = (long long)blockIdx.x * kPackSites;
+    const int n = (int)min((long long)kPackSites, V - base);
+    if (PACK) {
+        for (int j = threadIdx.x; j < n * 12; j += kPackSites) tile[j] = src[base * 12 + j];
+        __syncthreads();
+        if ((int)threadIdx.x < n)
+#pragma unroll
+            for (int c = 0; c < 12; c++) dst[(long long)c * V + base + threadIdx.x] = tile[threadIdx.x * 12 + c];
+    } else {
+        if ((int)threadIdx.x < n)
+#pragma unroll
+            for (int c = 0; c < 12; c++) tile[threadIdx.x * 12 + c] = src[(long long)c * V + base + threadIdx.x];
+        __syncthreads();
+        for (int j = threadIdx.x; j < n * 12; j += kPackSites) dst[base * 12 + j] = tile[j];
+    }
+}
+
+int launch_pack(ov_ctx* ctx, const double2* canonical, double2* abi) {
+    const long long V = ctx->lat.V;
+    pack_kernel<true><<<(unsigned)((V + kPackSites - 1) / kPackSites), kPackSites, 0, ctx->stream>>>(canonical, abi, V);
+    ctx->launches++;
+    OV_CUDA(ctx, cudaGetLastError());
+    return OV_OK;
+}
+int launch_unpack(ov_ctx* ctx, const double2* abi, double2* canonical) {
+    const long long V = ctx->lat.V;
+    pack_kernel<false><<<(unsigned)((V + kPackSites - 1) / kPackSites), kPackSites, 0, ctx->stream>>>(abi, canonical, V);
+    ctx->launches++;
+    OV_CUDA(ctx, cudaGetLastError());
+    return OV_OK;
+}
+
+// ------------------------------------------------------------------------------------------ BLAS-1
+constexpr int kEw = 4;  // complex elements per thread in elementwise kernels
+constexpr int kEwThreads = 256;
+
+__global__ void __launch_bounds__(kEwThreads) axpy_kernel(double2 a, const double2* __restrict__ x,
+                                                          double2* __restrict__ y, long long n) {
+    const long long base = (long long)blockIdx.x * (kEwThreads * kEw) + threadIdx.x;
+    double2 xv[kEw], yv[kEw];
+#pragma unroll
+    for (int m = 0; m < kEw; m++) {
+        const long long e = base + (long long)m * kEwThreads;
+        if (e < n) { xv[m] = x[e]; yv[m] = y[e]; }
+    }
+#pragma unroll
+    for (int m = 0; m < kEw; m++) {
+        const long long e = base + (long long)m * kEwThreads;
+        if (e < n) { cmadd(yv[m], a, xv[m]); y[e] = yv[m]; }
+    }
+}
+
+// z = a x + b y (a, b real); x or y may be null (treated as zero); z may alias x or y
+__global__ void __launch_bounds__(kEwThreads) axpby_kernel(double a, const double2* __restrict__ x, double b,
+                                                           const double2* __restrict__ y, double2* z,
+                                                           long long n) {
+    const long long base = (long long)blockIdx.x * (kEwThreads * kEw) + threadIdx.x;
+#pragma unroll
+    for (int m = 0; m < kEw; m++) {
+        const long long e = base + (long long)m * kEwThreads;
+        if (e < n) {
+            double2 v = make_double2(0.0, 0.0);
+            if (x) { const double2 w = x[e]; v.x = a * w.x; v.y = a * w.y; }
+            if (y) { const double2 w = y[e]; v.x = fma(b, w.x, v.x); v.y = fma(b, w.y, v.y); }
+            z[e] = v;
+        }
+    }
+}
+
+// y = gamma5 x : components 6..11 (spins 2,3) change sign.  n = 12 V, element e has component e / V.
+__global__ void __launch_bounds__(kEwThreads) gamma5_kernel(const double2* x, double2* y, long long V) {
+    const long long n = 12 * V;
+    const long long base = (long long)blockIdx.x * (kEwThreads * kEw) + threadIdx.x;
+#pragma unroll
+    for (int m = 0; m < kEw; m++) {
+        const long long e = base + (long long)m * kEwThreads;
+        if (e < n) {
+            double2 v = x[e];
+            if (e >= 6 * V) { v.x = -v.x; v.y = -v.y; }
+            y[e] = v;
+        }
+    }
+}
+
+static inline unsigned ew_blocks(long long n) { return (unsigned)((n + kEwThreads * kEw - 1) / (kEwThreads * kEw)); }
+
+int launch_axpy(ov_ctx* ctx, double2 a, const double2* x, double2* y) {
+    const long long n = (long long)spinor_elems(ctx);
+    axpy_kernel<<<ew_blocks(n), kEwThreads, 0, ctx->stream>>>(a, x, y, n);
+    ctx->launches++;
+    OV_CUDA(ctx, cudaGetLastError());
+    return OV_OK;
+}
+int launch_axpby(ov_ctx* ctx, double a, const double2* x, double b, const double2* y, double2* z) {
+    const long long n = (long long)spinor_elems(ctx);
+    axpby_kernel<<<ew_blocks(n), kEwThreads, 0, ctx->stream>>>(a, x, b, y, z, n);
+    ctx->launches++;
+    OV_CUDA(ctx, cudaGetLastError());
+    return OV_OK;
+}
+int launch_scale(ov_ctx* ctx, double a, double2* x) { return launch_axpby(ctx, a, x, 0.0, nullptr, x); }
+int launch_copy(ov_ctx* ctx, const double2* x, double2* y) { return launch_axpby(ctx, 1.0, x, 0.0, nullptr, y); }
+int launch_zero(ov_ctx* ctx, double2* x) {
+    OV_CUDA(ctx, cudaMemsetAsync(x, 0, spinor_elems(ctx) * sizeof(double2), ctx->stream));
+    return OV_OK;
+}
+int launch_gamma5(ov_ctx* ctx, const double2* x, double2* y) {
+    const long long n = (long long)spinor_elems(ctx);
+    gamma5_kernel<<<ew_blocks(n), kEwThreads, 0, ctx->stream>>>(x, y, ctx->lat.V);
+    ctx->launches++;
+    OV_CUDA(ctx, cudaGetLastError());
+    return OV_OK;
+}
+
+// ------------------------------------------------------------------------------------------ reductions
+// multi-dot: r_j = sum_e conj(x_j[e]) y[e], j < nvec.  Each warp owns kDotE*32 consecutive elements of y,
+// keeps them in registers, and streams the same window of every x_j once: y is read from HBM exactly
+// once however many vectors there are (the small-space V^+ x of PAPER.md:39/:81 with k = 100-200).
+constexpr int kDotE = 8;
+constexpr int kDotThreads = 256;
+constexpr int kDotWarpElems = kDotE * 32;
+
+__global__ void __launch_bounds__(kDotThreads) multi_dot_kernel(const double2* __restrict__ xs, size_t stride,
+                                                                int nvec, const double2* __restrict__ y,
+                                                                long long n, long long nwarps,
+                                                                double2* __restrict__ partial) {
+    const int lane = threadIdx.x & 31;
+    const long long warp = (long long)blockIdx.x * (kDotThreads / 32) + (threadIdx.x >> 5);
+    if (warp >= nwarps) return;
+    const long long base = warp * kDotWarpElems + lane;
+    double2 yv[kDotE];
+#pragma unroll
+    for (int m = 0; m < kDotE; m++) {
+        const long long e = base + m * 32;
+        yv[m] = (e < n) ? y[e] : make_double2(0.0, 0.0);
+    }
+    for (int j = 0; j < nvec; j++) {
+        const double2* x = xs + (size_t)j * stride;
+        double2 xv[kDotE];
+#pragma unroll
+        for (int m = 0; m < kDotE; m++) {
+            const long long e = base + m * 32;
+            xv[m] = (e < n) ? __ldcs(x + e) : make_double2(0.0, 0.0);
+        }
+        double2 acc = make_double2(0.0, 0.0);
+#pragma unroll
+        for (int m = 0; m < kDotE; m++) cmaddc(acc, xv[m], yv[m]);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            acc.x += __shfl_xor_sync(0xffffffffu, acc.x, o);
+            acc.y += __shfl_xor_sync(0xffffffffu, acc.y, o);
+        }
+        if (lane == 0) partial[(long long)j * nwarps + warp] = acc;
+    }
+}
+
+// one block per result: fixed-order strided accumulation then a fixed shared-memory tree
+constexpr int kRedThreads = 256;
+__global__ void __launch_bounds__(kRedThreads) reduce_partials_kernel(const double2* __restrict__ partial,
+                                                                      long long nwarps, double2* __restrict__ result) {
+    __shared__ double2 sh[kRedThreads];
+    const double2* p = partial + (long long)blockIdx.x * nwarps;
+    double2 acc = make_double2(0.0, 0.0);
+    for (long long w = threadIdx.x; w < nwarps; w += kRedThreads) acc = cadd(acc, p[w]);
+    sh[threadIdx.x] = acc;
+    __syncthreads();
+    for (int o = kRedThreads / 2; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) sh[threadIdx.x] = cadd(sh[threadIdx.x], sh[threadIdx.x + o]);
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) result[blockIdx.x] = sh[0];
+}
+
+int launch_multi_dot(ov_ctx* ctx, const double2* xs, size_t stride, int nvec, const double2* y) {
+    const long long n = (long long)spinor_elems(ctx);
+    const long long nwarps = (n + kDotWarpElems - 1) / kDotWarpElems;
+    OV_TRY(ensure_reduction_buffers(ctx, (size_t)nwarps * nvec, (size_t)nvec));
+    const unsigned blocks = (unsigned)((nwarps + kDotThreads / 32 - 1) / (kDotThreads / 32));
+    multi_dot_kernel<<<blocks, kDotThreads, 0, ctx->stream>>>(xs, stride, nvec, y, n, nwarps, ctx->d_partial);
+    reduce_partials_kernel<<<nvec, kRedThreads, 0, ctx->stream>>>(ctx->d_partial, nwarps, ctx->d_result);
+    ctx->launches += 2;
+    OV_CUDA(ctx, cudaGetLastError());
+    return OV_OK;
+}
+
+int fetch_results(ov_ctx* ctx, int n, double2* host_out) {
+    OV_CUDA(ctx, cudaMemcpyAsync(ctx->h_result, ctx->d_result, (size_t)n * sizeof(double2),
+                                 cudaMemcpyDeviceToHost, ctx->stream));
+    OV_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    for (int i = 0; i < n; i++) host_out[i] = ctx->h_result[i];
+    return OV_OK;
+}
+
+int dot_host(ov_ctx* ctx, const double2* x, const double2* y, double2* out) {
+    OV_TRY(launch_multi_dot(ctx, x, 0, 1, y));
+    return fetch_results(ctx, 1, out);
+}
+int norm2_host(ov_ctx* ctx, const double2* x, double* out) {
+    double2 r;
+    OV_TRY(dot_host(ctx, x, x, &r));
+    *out = r.x;
+    return OV_OK;
+}
+
+// ------------------------------------------------------------------------------------------ multi-axpy
+// out_j = bscale_j * base + sum_{i<nvec} C[i*J + j] * x_i   for j < J  (J outputs per pass over the x_i).
+// The coefficient block sits in shared memory; every x_i element is read once per pass.
+constexpr int kMaThreads = 256;
+template <int J>
+__global__ void __launch_bounds__(kMaThreads) multi_axpy_kernel(const double2* __restrict__ xs, size_t stride,
+                                                                int nvec, const double2* __restrict__ C,
+                                                                const double2* base,
+                                                                const MultiAxpyOuts o, long long n) {
+    extern __shared__ double2 shC[];
+    for (int q = threadIdx.x; q < nvec * J; q += kMaThreads) shC[q] = C[q];
+    __syncthreads();
+    const long long e = (long long)blockIdx.x * kMaThreads + threadIdx.x;
+    if (e >= n) return;
+    double2 acc[J];
+    const double2 b = base ? base[e] : make_double2(0.0, 0.0);
+#pragma unroll
+    for (int j = 0; j < J; j++) acc[j] = make_double2(o.bscale[j] * b.x, o.bscale[j] * b.y);
+    int i = 0;
+    for (; i + 4 <= nvec; i += 4) {
+        double2 xv[4];
+#pragma unroll
+        for (int u = 0; u < 4; u++) xv[u] = __ldcs(xs + (size_t)(i + u) * stride + e);
+#pragma unroll
+        for (int u = 0; u < 4; u++)
+#pragma unroll
+            for (int j = 0; j < J; j++) cmadd(acc[j], shC[(i + u) * J + j], xv[u]);
+    }
+    for (; i < nvec; i++) {
+        const double2 xv = __ldcs(xs + (size_t)i * stride + e);
+#pragma unroll
+        for (int j = 0; j < J; j++) cmadd(acc[j], shC[i * J + j], xv);
+    }
+#pragma unroll
+    for (int j = 0; j < J; j++) o.out[j][e] = acc[j];
+}
+
+// host wrapper used by the projector and the Lanczos Ritz rotation.
+// C_dev: nvec x J complex (row i, column j) on the device; o: J output pointers + base scales (by value).
+int launch_multi_axpy(ov_ctx* ctx, const double2* xs, size_t stride, int nvec, int J, const double2* C_dev,
+                      const double2* base, const MultiAxpyOuts& o) {
+    const long long n = (long long)spinor_elems(ctx);
+    const unsigned blocks = (unsigned)((n + kMaThreads - 1) / kMaThreads);
+    const size_t shmem = (size_t)nvec * J * sizeof(double2);
+    if (shmem > 200 * 1024) return fail(ctx, OV_EINVAL, "multi_axpy: coefficient block too large (%zu B)", shmem);
+#define OV_MA_CASE(JJ)                                                                                         \
+    case JJ:                                                                                                   \
+        if (shmem > 48 * 1024)                                                                                 \
+            OV_CUDA(ctx, cudaFuncSetAttribute(multi_axpy_kernel<JJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
+                                              (int)shmem));                                                    \
+        multi_axpy_kernel<JJ><<<blocks, kMaThreads, shmem, ctx->stream>>>(xs, stride, nvec, C_dev, base, o, n); \
+        break;
+    switch (J) {
+        OV_MA_CASE(1)
+        OV_MA_CASE(2)
+        OV_MA_CASE(4)
+        OV_MA_CASE(8)
+        default:
+            return fail(ctx, OV_EINVAL, "multi_axpy: J must be 1, 2, 4 or 8");
+    }
+#undef OV_MA_CASE
+    ctx->launches++;
+    OV_CUDA(ctx, cudaGetLastError());
+    return OV_OK;
+}
+
+}  // namespace ov

@@ -1,0 +1,122 @@
+// Multi-shift ("multi-mass") CG on A = D_ov(0)^+ D_ov(0) = gamma5 D_ov gamma5 D_ov (
+// PAPER.md:85; O8/G10).  One Krylov space serves all shifts sigma_i = m_i^2/(1 - m_i^2/4).
+// Host loop, device vectors; two host synchronisations per iteration (the scalars (p,q) and (r,r)),
+// negligible next to the ~2(2n+1) Wilson launches inside each A.
+#include <algorithm>
+#include <cmath>
+#include <numeric>
+
+#include "ov_internal.h"
+
+namespace ov {
+
+// out = A in  (tmp: one scratch spinor, none of the three may alias)
+static int apply_A(ov_ctx* ctx, const double2* in, double2* tmp, double2* out) {
+    OV_TRY(apply_dov(ctx, 0.0, in, tmp));
+    OV_TRY(launch_gamma5(ctx, tmp, tmp));
+    OV_TRY(apply_dov(ctx, 0.0, tmp, out));
+    return launch_gamma5(ctx, out, out);
+}
+
+}  // namespace ov
+
+using namespace ov;
+
+extern "C" int ov_multishift_cg(ov_ctx* ctx, const double* masses_host, int nmass, const void* b_, void* x_,
+                                double tol, int maxiter, int* iters_out, double* relres_out) {
+    if (!ctx) return OV_EINVAL;
+    if (!masses_host || nmass < 1 || nmass > 64 || !b_ || !x_ || !(tol > 0) || maxiter < 1)
+        return fail(ctx, OV_EINVAL, "bad argument to ov_multishift_cg");
+    if (ctx->order < 0) return fail(ctx, OV_ESTATE, "ov_set_polynomial has not been called");
+    const size_t n = spinor_elems(ctx), bytes = n * sizeof(double2);
+    const double2* b = (const double2*)b_;
+    double2* x = (double2*)x_;
+
+    std::vector<double> sig(nmass);
+    for (int i = 0; i < nmass; i++) {
+        const double m = masses_host[i];
+        if (!(m * m < 4.0)) return fail(ctx, OV_EINVAL, "mass %d out of range", i);
+        sig[i] = m * m / (1.0 - 0.25 * m * m);
+    }
+    std::vector<int> ord(nmass);
+    std::iota(ord.begin(), ord.end(), 0);
+    std::sort(ord.begin(), ord.end(), [&](int a, int c) { return sig[a] < sig[c]; });
+    const double s0 = sig[ord[0]];
+
+    // device vectors: p_i (nmass), r, q, tmp
+    double2* pool = nullptr;
+    OV_CUDA(ctx, cudaMalloc(&pool, bytes * (size_t)(nmass + 3)));
+    struct Free { double2* p; ~Free() { cudaFree(p); } } guard{pool};
+    std::vector<double2*> p(nmass);
+    for (int i = 0; i < nmass; i++) p[i] = pool + (size_t)i * n;
+    double2* r = pool + (size_t)nmass * n;
+    double2* q = r + n;
+    double2* tmp = q + n;
+
+    for (int i = 0; i < nmass; i++) {
+        OV_TRY(launch_zero(ctx, x + (size_t)i * n));
+        OV_TRY(launch_copy(ctx, b, p[i]));
+    }
+    OV_TRY(launch_copy(ctx, b, r));
+    double rr;
+    OV_TRY(norm2_host(ctx, r, &rr));
+    const double bnorm = std::sqrt(rr);
+    if (bnorm == 0.0) {
+        if (iters_out) *iters_out = 0;
+        if (relres_out) for (int i = 0; i < nmass; i++) relres_out[i] = 0.0;
+        return OV_OK;
+    }
+    std::vector<double> zeta(nmass, 1.0), zeta_old(nmass, 1.0), zeta_new(nmass);
+    std::vector<char> active(nmass, 1);
+    double a_old = 1.0, beta_old = 0.0;
+    int it = 0;
+    bool converged = false;
+    while (it < maxiter) {
+        // q = (A + s0) p_0   (position 0 = smallest shift)
+        OV_TRY(apply_A(ctx, p[0], tmp, q));
+        if (s0 != 0.0) OV_TRY(launch_axpy(ctx, make_double2(s0, 0.0), p[0], q));
+        double2 pq;
+        OV_TRY(dot_host(ctx, p[0], q, &pq));
+        const double a = rr / pq.x;
+        for (int j = 0; j < nmass; j++) {
+            const double s = sig[ord[j]] - s0;
+            zeta_new[j] = zeta[j] * zeta_old[j] * a_old /
+                          (a * beta_old * (zeta_old[j] - zeta[j]) + zeta_old[j] * a_old * (1.0 + s * a));
+        }
+        for (int j = 0; j < nmass; j++)
+            if (active[j])
+                OV_TRY(launch_axpy(ctx, make_double2(a * zeta_new[j] / zeta[j], 0.0), p[j], x + (size_t)ord[j] * n));
+        OV_TRY(launch_axpy(ctx, make_double2(-a, 0.0), q, r));
+        double rr_new;
+        OV_TRY(norm2_host(ctx, r, &rr_new));
+        const double beta = rr_new / rr;
+        for (int j = 0; j < nmass; j++)
+            if (active[j]) {
+                const double ratio = zeta_new[j] / zeta[j];
+                OV_TRY(launch_axpby(ctx, zeta_new[j], r, beta * ratio * ratio, p[j], p[j]));
+            }
+        zeta_old = zeta;
+        zeta = zeta_new;
+        a_old = a;
+        beta_old = beta;
+        rr = rr_new;
+        it++;
+        for (int j = 1; j < nmass; j++)
+            if (active[j] && std::fabs(zeta[j]) * std::sqrt(rr) <= tol * bnorm) active[j] = 0;
+        if (std::sqrt(rr) <= tol * bnorm) { converged = true; break; }
+    }
+    if (iters_out) *iters_out = it;
+    if (relres_out) {  // true residuals |b - (A + sigma_i) x_i| / |b|
+        for (int i = 0; i < nmass; i++) {
+            OV_TRY(apply_A(ctx, x + (size_t)i * n, tmp, q));
+            OV_TRY(launch_axpy(ctx, make_double2(sig[i], 0.0), x + (size_t)i * n, q));
+            OV_TRY(launch_axpby(ctx, 1.0, b, -1.0, q, q));
+            double e;
+            OV_TRY(norm2_host(ctx, q, &e));
+            relres_out[i] = std::sqrt(e) / bnorm;
+        }
+    }
+    OV_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    if (!converged) return fail(ctx, OV_ENOCONV, "multi-shift CG: %d iterations without reaching tol", it);
+    return OV_OK;
+}

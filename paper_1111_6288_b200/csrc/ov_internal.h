@@ -1,0 +1,135 @@
+// Internal declarations shared by the translation units of libov.so (CUDA side only).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdarg>
+#include <cstdio>
+#include <string>
+#include <vector>
+
+#include "ov.h"
+
+namespace ov {
+
+constexpr int kSpinorComplex = 12;  // 4 spins x 3 colours
+
+struct Lattice {
+    int X, Y, Z, T;
+    long long V;  // sites
+};
+
+// Epilogue of the Wilson kernel:  out = s * G (in - kappa * hop(in)) + a1*A1 + a2*A2 + a3*A3
+//   G = gamma5 (g5 = 1) or the identity (g5 = 0);  hop_only: out = hop(in)  (no diagonal term, no axpy)
+// A1..A3 are optional ABI spinors read at the output site only, so `out` may alias any of them.
+struct Epilogue {
+    double s = 1.0;
+    int g5 = 1;
+    int hop_only = 0;
+    const double2* A1 = nullptr;
+    const double2* A2 = nullptr;
+    const double2* A3 = nullptr;
+    double a1 = 0.0, a2 = 0.0, a3 = 0.0;
+    int a_g5 = 0;  // bit k-1 set: operand A_k enters as gamma5 A_k
+};
+
+}  // namespace ov
+
+struct ov_ctx {
+    ov::Lattice lat{};
+    double kappa = 0.0;
+    int recon = 18;
+    cudaStream_t stream = nullptr;
+    double2* gauge = nullptr;  // [mu][recon/2][V] double2
+    int dslash_variant = 0;
+    long long launches = 0;
+    mutable std::string err;
+
+    // polynomial
+    std::vector<double> coef;
+    int order = -1;
+    double eps = 0.0, norm = 0.0;
+
+    // small space (borrowed V)
+    const double2* Vlow = nullptr;
+    std::vector<double> lambda;
+    int k = 0;
+    double* d_sgn = nullptr;       // k doubles: sign(lambda_i)
+    double2* d_coef = nullptr;     // k complex: c = V^+ x
+    int cap_k = 0;
+
+    // workspaces
+    double2* ws[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    double2* d_partial = nullptr;  // reduction partials
+    size_t partial_cap = 0;        // in double2
+    double2* d_result = nullptr;   // reduced results (device)
+    size_t result_cap = 0;
+    double2* h_result = nullptr;   // pinned host mirror
+    double2* host_stage_in = nullptr;   // device staging for *_host calls (canonical)
+    double2* host_stage_abi = nullptr;
+    double2* host_stage_out = nullptr;
+};
+
+namespace ov {
+
+int fail(const ov_ctx* ctx, int code, const char* fmt, ...);
+int cuda_fail(const ov_ctx* ctx, cudaError_t e, const char* what);
+
+#define OV_CUDA(ctx, call)                                         \
+    do {                                                           \
+        cudaError_t e__ = (call);                                  \
+        if (e__ != cudaSuccess) return ov::cuda_fail(ctx, e__, #call); \
+    } while (0)
+
+#define OV_TRY(call)                 \
+    do {                             \
+        int rc__ = (call);           \
+        if (rc__ != OV_OK) return rc__; \
+    } while (0)
+
+inline size_t spinor_elems(const ov_ctx* c) { return (size_t)kSpinorComplex * (size_t)c->lat.V; }
+
+// workspace spinor i (allocated on first use)
+int workspace(ov_ctx* ctx, int i, double2** out);
+int ensure_reduction_buffers(ov_ctx* ctx, size_t partial_elems, size_t result_elems);
+
+// --- kernels (launchers); all enqueue on ctx->stream and bump ctx->launches ---
+int launch_gauge_relayout(ov_ctx* ctx, const double2* canonical);
+int launch_pack(ov_ctx* ctx, const double2* canonical, double2* abi);
+int launch_unpack(ov_ctx* ctx, const double2* abi, double2* canonical);
+int launch_wilson(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep);
+int launch_wilson_gather(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep);
+int launch_wilson_tiled(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep);
+bool tiled_supported(const ov_ctx* ctx);
+// host-side dense Hermitian eigensolver (cyclic complex Jacobi): A (n x n, row-major complex, destroyed),
+// w ascending, Z row-major with eigenvectors as COLUMNS
+void host_eigh(int n, std::vector<double2>& A, std::vector<double>& w, std::vector<double2>& Z);
+
+// BLAS-1 on ABI spinors (n = 12 V complex)
+int launch_axpy(ov_ctx* ctx, double2 a, const double2* x, double2* y);                     // y += a x
+int launch_axpby(ov_ctx* ctx, double a, const double2* x, double b, const double2* y, double2* z);  // z = a x + b y
+int launch_scale(ov_ctx* ctx, double a, double2* x);
+int launch_copy(ov_ctx* ctx, const double2* x, double2* y);
+int launch_zero(ov_ctx* ctx, double2* x);
+int launch_gamma5(ov_ctx* ctx, const double2* x, double2* y);  // y = gamma5 x (may alias)
+// nvec dots <x_j, y> for j < nvec, x_j = xs + j*stride (complex results on device in ctx->d_result[0..nvec))
+int launch_multi_dot(ov_ctx* ctx, const double2* xs, size_t stride, int nvec, const double2* y);
+int fetch_results(ov_ctx* ctx, int n, double2* host_out);  // sync + copy d_result[0..n) to host
+int dot_host(ov_ctx* ctx, const double2* x, const double2* y, double2* out);
+int norm2_host(ov_ctx* ctx, const double2* x, double* out);
+// out_j = bscale_j * base + sum_{i<nvec} C[i*J+j] x_i, j < J in {1,2,4,8}; C (nvec x J complex) on the device
+struct MultiAxpyOuts {
+    double2* out[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    double bscale[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+};
+int launch_multi_axpy(ov_ctx* ctx, const double2* xs, size_t stride, int nvec, int J, const double2* C_dev,
+                      const double2* base, const MultiAxpyOuts& o);
+
+// projector: c = V^+ x (left in ctx->d_result[0..k)); perp = x - V c; low = V (sgn o c)
+int project(ov_ctx* ctx, const double2* x, double2* perp, double2* low);
+
+// operator drivers
+int sign_poly(ov_ctx* ctx, const double2* x, double2* out, const Epilogue& fin);
+int apply_sign(ov_ctx* ctx, const double2* in, double2* out);
+int apply_dov(ov_ctx* ctx, double mass, const double2* in, double2* out);
+
+}  // namespace ov

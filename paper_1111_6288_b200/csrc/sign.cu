@@ -1,0 +1,117 @@
+// sign(H_w) and D_ov drivers.
+//
+//   sign(H_w) x  =  sum_i sign(lambda_i) v_i (v_i^+ x)   +   Q P(Q^2) (1 - V V^+) x
+//   P(Q^2) = sum_j c_j T_j(z),  z = (2Q^2 - 1 - eps)/(1 - eps), evaluated by the Clenshaw recurrence with
+//   alpha = 4/(1-eps), beta = 2(1+eps)/(1-eps):   b_j = c_j x + alpha Q(Q b_{j+1}) - beta b_{j+1} - b_{j+2}
+//   Every Clenshaw order is exactly two launches of the Wilson kernel: the first with epilogue
+//   gamma5 * (1/norm), the second with gamma5 * (alpha/norm) plus the three-vector axpy written in place
+//   over b_{j+2} -- no separate BLAS-1 pass touches HBM inside the recurrence.
+#include "ov_internal.h"
+
+namespace ov {
+
+// C[i*2+0] = -c_i ; C[i*2+1] = sgn_i * c_i     (c = V^+ x sits in d_result after the multi-dot)
+__global__ void projector_coef_kernel(const double2* __restrict__ c, const double* __restrict__ sgn, int k,
+                                      double2* __restrict__ C) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= k) return;
+    const double2 v = c[i];
+    const double s = sgn[i];
+    C[2 * i + 0] = make_double2(-v.x, -v.y);
+    C[2 * i + 1] = make_double2(s * v.x, s * v.y);
+}
+
+// c = V^+ x ; perp = x - V c ; low = V (sign(lambda) o c).  Two passes over V ("D_ov requires
+// all of the H_w eigenvectors for each matrix multiplication"): 2 k 192 B/site + 4 spinors.
+int project(ov_ctx* ctx, const double2* x, double2* perp, double2* low) {
+    const size_t stride = spinor_elems(ctx);
+    OV_TRY(launch_multi_dot(ctx, ctx->Vlow, stride, ctx->k, x));
+    projector_coef_kernel<<<(ctx->k + 127) / 128, 128, 0, ctx->stream>>>(ctx->d_result, ctx->d_sgn, ctx->k, ctx->d_coef);
+    ctx->launches++;
+    OV_CUDA(ctx, cudaGetLastError());
+    MultiAxpyOuts o;
+    o.out[0] = perp; o.bscale[0] = 1.0;
+    o.out[1] = low;  o.bscale[1] = 0.0;
+    return launch_multi_axpy(ctx, ctx->Vlow, stride, ctx->k, 2, ctx->d_coef, x, o);
+}
+
+// out = fin.s * G [Q P(Q^2) x]-ish: the last Wilson launch (result = Q y) carries `fin`:
+//   out = (fin.s / norm) * G (y - kappa hop y) + fin.a1 A1 + fin.a2 A2 + fin.a3 A3
+// with fin.g5 = 1 -> G = gamma5 (plain sign), fin.g5 = 0 -> G = 1 (gamma5 * sign, for D_ov).
+int sign_poly(ov_ctx* ctx, const double2* x, double2* out, const Epilogue& fin) {
+    if (ctx->order < 0) return fail(ctx, OV_ESTATE, "ov_set_polynomial has not been called");
+    const int n = ctx->order;
+    const double* c = ctx->coef.data();
+    const double eps = ctx->eps, inv = 1.0 / ctx->norm;
+    const double alpha = 4.0 / (1.0 - eps), beta = 2.0 * (1.0 + eps) / (1.0 - eps);
+    double2 *b1, *b2, *t;
+    OV_TRY(workspace(ctx, 0, &b1));
+    OV_TRY(workspace(ctx, 1, &b2));
+    OV_TRY(workspace(ctx, 2, &t));
+
+    const double2* y = nullptr;
+    if (n == 0) {
+        OV_TRY(launch_axpby(ctx, c[0], x, 0.0, nullptr, b1));
+        y = b1;
+    } else {
+        // b_n = c_n x  (b_{n+1} = b_{n+2} = 0)
+        OV_TRY(launch_axpby(ctx, c[n], x, 0.0, nullptr, b1));
+        bool b2_valid = false;
+        for (int j = n - 1; j >= 0; j--) {
+            Epilogue e1;  // t = Q b1
+            e1.s = inv;
+            e1.g5 = 1;
+            OV_TRY(launch_wilson(ctx, b1, t, e1));
+            Epilogue e2;  // b2 <- f*(alpha Q t - beta b1) + c_j x - b2 ; f = 1 (j >= 1) or 1/2 (j = 0)
+            const double f = (j == 0) ? 0.5 : 1.0;
+            e2.s = f * alpha * inv;
+            e2.g5 = 1;
+            e2.A1 = x;  e2.a1 = c[j];
+            e2.A2 = b1; e2.a2 = -f * beta;
+            if (b2_valid) { e2.A3 = b2; e2.a3 = -1.0; }
+            OV_TRY(launch_wilson(ctx, t, b2, e2));
+            b2_valid = true;
+            double2* tmp = b1; b1 = b2; b2 = tmp;
+        }
+        y = b1;  // after the j = 0 step b1 holds y
+    }
+    Epilogue ef = fin;
+    ef.s = fin.s * inv;
+    ef.hop_only = 0;
+    return launch_wilson(ctx, y, out, ef);
+}
+
+int apply_sign(ov_ctx* ctx, const double2* in, double2* out) {
+    Epilogue fin;
+    fin.s = 1.0;
+    fin.g5 = 1;
+    if (ctx->k > 0) {
+        double2 *perp, *low;
+        OV_TRY(workspace(ctx, 3, &perp));
+        OV_TRY(workspace(ctx, 4, &low));
+        OV_TRY(project(ctx, in, perp, low));
+        fin.A1 = low; fin.a1 = 1.0;
+        return sign_poly(ctx, perp, out, fin);
+    }
+    return sign_poly(ctx, in, out, fin);
+}
+
+// D_ov(m) x = (1 + m/2) x + (1 - m/2) gamma5 sign(H_w) x ; gamma5 * [gamma5 D_w y / norm] = D_w y / norm, so the
+// final Wilson launch runs with G = 1 and the x / gamma5 x_low terms ride in its epilogue (row a5).
+int apply_dov(ov_ctx* ctx, double mass, const double2* in, double2* out) {
+    Epilogue fin;
+    fin.s = 1.0 - 0.5 * mass;
+    fin.g5 = 0;
+    fin.A1 = in; fin.a1 = 1.0 + 0.5 * mass;
+    if (ctx->k > 0) {
+        double2 *perp, *low;
+        OV_TRY(workspace(ctx, 3, &perp));
+        OV_TRY(workspace(ctx, 4, &low));
+        OV_TRY(project(ctx, in, perp, low));
+        fin.A2 = low; fin.a2 = 1.0 - 0.5 * mass; fin.a_g5 = 2;
+        return sign_poly(ctx, perp, out, fin);
+    }
+    return sign_poly(ctx, in, out, fin);
+}
+
+}  // namespace ov

@@ -1,0 +1,239 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs.  Tolerances (BASELINE.json north_star): rel-L2 <= 1e-12 per Wilson apply,
+<= 1e-10 per sign / D_ov apply.  Run on the B200 box with  pytest -m gpu.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from oracle import chebyshev as ch
+from oracle import dense
+from oracle.multishift_cg import multishift_cg, sigma_of_mass
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+KAPPA = 0.19
+NORM = 1.0 + 8.0 * KAPPA
+TOL_HW = 1e-12
+TOL_DOV = 1e-10
+
+
+def rel(a, b):
+    return np.linalg.norm((a - b).ravel()) / np.linalg.norm(b.ravel())
+
+
+@pytest.fixture(scope="module")
+def ovp():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_1111_6288_b200 as m
+    from paper_1111_6288_b200 import build
+    build.build()
+    return m
+
+
+def make(ovp, dims, U, recon=18, variant=0):
+    op = ovp.Overlap(dims, KAPPA, U, recon=recon)
+    if variant:
+        op.set_dslash_variant(variant)
+    return op
+
+
+def to_dev(op, x):
+    return op.pack_spinor(torch.from_numpy(np.ascontiguousarray(x)).cuda())
+
+
+def to_host(op, x):
+    return op.unpack_spinor(x).cpu().numpy()
+
+
+def variants(op_dims):
+    return [1, 2]
+
+
+# ------------------------------------------------------------------------------------------ layout
+def test_pack_unpack_roundtrip(ovp):
+    dims = (4, 2, 6, 8)
+    op = make(ovp, dims, wl.unit_links(dims))
+    x = np.stack([wl.gaussian_source(dims, s) for s in (1, 2, 3)])
+    d = to_dev(op, x)
+    assert d.shape == (3, 12, op.V)
+    # ABI layout: component (3*s+c) of site i at [comp][i]
+    ref = x.reshape(3, op.V, 12).transpose(0, 2, 1)
+    assert np.array_equal(d.cpu().numpy(), ref)
+    assert np.array_equal(to_host(op, d), x)
+
+
+# ------------------------------------------------------------------------------------------ Wilson kernel
+@pytest.mark.parametrize("dims,spread", [((4, 4, 4, 4), 0.3), ((4, 2, 6, 8), 0.6), ((8, 8, 8, 16), 0.5),
+                                         ((24, 4, 4, 2), 0.8), ((6, 10, 2, 4), 0.4)])
+@pytest.mark.parametrize("recon", [18, 12])
+def test_dslash_and_hw_vs_oracle(ovp, dims, spread, recon):
+    U = wl.su3_links(dims, spread, wl.gauge_seed(1))
+    nsrc = 3
+    x = np.stack([wl.gaussian_source(dims, wl.source_seed(1, j)) for j in range(nsrc)])
+    ref_hop = np.stack([oracle.wilson_hop(dims, U, v) for v in x])
+    ref_hw = np.stack([oracle.hw(dims, KAPPA, U, v) for v in x])
+    op = make(ovp, dims, U, recon)
+    tested = 0
+    for variant in (1, 2):
+        try:
+            op.set_dslash_variant(variant)
+        except ovp.OvError:
+            continue
+        tested += 1
+        d = to_dev(op, x)
+        assert rel(to_host(op, op.dslash(d)), ref_hop) <= TOL_HW
+        got = to_host(op, op.apply_hw(d))
+        assert rel(got, ref_hw) <= TOL_HW
+        for j in range(nsrc):
+            assert rel(got[j], ref_hw[j]) <= TOL_HW
+    assert tested >= 1
+
+
+def test_hw_rejects_aliasing_and_bad_args(ovp):
+    dims = (4, 4, 4, 4)
+    op = make(ovp, dims, wl.unit_links(dims))
+    x = op.new_spinor()
+    with pytest.raises(ovp.OvError):
+        op.apply_hw(x, out=x)
+    with pytest.raises(ovp.OvError):
+        op.apply_sign(x)  # no polynomial set
+    with pytest.raises(ovp.OvError):
+        op.set_polynomial([1.0, 0.5], 0.0, NORM)
+    V = op.new_spinor(2)
+    op.set_polynomial([1.0, 0.5], 0.01, NORM)
+    with pytest.raises(ovp.OvError):
+        op.set_smallspace(V, [0.1, 0.0])  # sign(0) undefined
+
+
+def test_hw_host_entry_point(ovp):
+    dims = (4, 2, 6, 8)
+    U = wl.su3_links(dims, 0.5, 5)
+    x = np.stack([wl.gaussian_source(dims, 6), wl.gaussian_source(dims, 7)])
+    op = make(ovp, dims, U)
+    got = op.apply_hw_host(x)
+    ref = np.stack([oracle.hw(dims, KAPPA, U, v) for v in x])
+    assert rel(got, ref) <= TOL_HW
+
+
+# ------------------------------------------------------------------------------------------ BLAS-1
+def test_blas(ovp):
+    dims = (6, 10, 2, 4)  # 12*480 = 5760 elements: several warps plus a ragged tail
+    op = make(ovp, dims, wl.unit_links(dims))
+    x = wl.gaussian_source(dims, 1)
+    y = wl.gaussian_source(dims, 2)
+    dx, dy = to_dev(op, x), to_dev(op, y)
+    d = op.blas_dot(dx, dy)
+    assert abs(d - np.vdot(x, y)) <= 1e-13 * np.linalg.norm(x) * np.linalg.norm(y)
+    assert abs(op.blas_norm2(dx) - np.vdot(x, x).real) <= 1e-13 * np.vdot(x, x).real
+    assert op.blas_dot(dx, dy) == d  # bit-reproducible
+    a = 0.3 - 1.7j
+    op.blas_axpy(a, dx, dy)
+    assert rel(to_host(op, dy), y + a * x) <= 1e-15
+    op.blas_scale(-2.5, dx)
+    assert rel(to_host(op, dx), -2.5 * x) <= 1e-15
+
+
+# ------------------------------------------------------------------------------------------ config 0: 4^4
+@pytest.fixture(scope="module")
+def cfg0():
+    cfg = wl.CONFIGS[0]
+    U = wl.su3_links(cfg.dims, cfg.spread, wl.gauge_seed(0))
+    w, Zv, _, _ = dense.eig_hw(cfg.dims, cfg.kappa, U)
+    x = wl.gaussian_source(cfg.dims, wl.source_seed(0, 0))
+    V, lam = dense.lowest_modes(w, Zv, cfg.norm, cfg.k, x.shape)
+    return dict(cfg=cfg, U=U, w=w, Z=Zv, x=x, V=V, lam=lam)
+
+
+def setup_op(ovp, c, recon=18, variant=0, with_small=True):
+    cfg = c["cfg"]
+    op = make(ovp, cfg.dims, c["U"], recon, variant)
+    coef = ovp.chebyshev_coeffs(cfg.order, cfg.eps)
+    op.set_polynomial(coef, cfg.eps, cfg.norm)
+    if with_small:
+        op.set_smallspace(to_dev(op, c["V"]), c["lam"])
+    return op, coef
+
+
+def test_projector_vs_numpy(ovp, cfg0):
+    op, _ = setup_op(ovp, cfg0)
+    x = cfg0["x"]
+    V = cfg0["V"].reshape(len(cfg0["lam"]), -1)
+    c = V.conj() @ x.ravel()
+    perp, low, coef = op.project(to_dev(op, x))
+    assert np.max(np.abs(coef - c)) <= 1e-13 * np.linalg.norm(x)
+    assert rel(to_host(op, perp), (x.ravel() - c @ V).reshape(x.shape)) <= 1e-13
+    assert rel(to_host(op, low), ((np.sign(cfg0["lam"]) * c) @ V).reshape(x.shape)) <= 1e-13
+
+
+@pytest.mark.parametrize("recon", [18, 12])
+@pytest.mark.parametrize("with_small", [True, False])
+def test_config0_sign_and_dov(ovp, cfg0, recon, with_small):
+    c = cfg0
+    cfg = c["cfg"]
+    op, coef = setup_op(ovp, c, recon, with_small=with_small)
+    V, lam = (c["V"], c["lam"]) if with_small else (None, None)
+    x = c["x"]
+    dx = to_dev(op, x)
+    ref_s = oracle.sign(cfg.dims, cfg.kappa, c["U"], coef, cfg.eps, cfg.norm, V, lam, x)
+    assert rel(to_host(op, op.apply_sign(dx)), ref_s) <= TOL_DOV
+    for mass in (0.0, 0.1):
+        ref_d = oracle.dov(cfg.dims, cfg.kappa, c["U"], coef, cfg.eps, cfg.norm, V, lam, mass, x)
+        assert rel(to_host(op, op.apply_dov(mass, dx)), ref_d) <= TOL_DOV
+    # and against the exact dense sign, within the polynomial's own error (reading G15)
+    exact = dense.exact_sign_apply(c["w"], c["Z"], x)
+    assert rel(to_host(op, op.apply_sign(dx)), exact) <= ch.delta_measured(coef, cfg.eps)
+    got_host = op.apply_dov_host(0.0, x)
+    assert rel(got_host, oracle.dov(cfg.dims, cfg.kappa, c["U"], coef, cfg.eps, cfg.norm, V, lam, 0.0, x)) <= TOL_DOV
+
+
+def test_degenerate_orders(ovp, cfg0):
+    c = cfg0
+    cfg = c["cfg"]
+    op = make(ovp, cfg.dims, c["U"])
+    dx = to_dev(op, c["x"])
+    for n in (0, 1, 2):
+        coef = ovp.chebyshev_coeffs(n, 0.04)
+        op.set_polynomial(coef, 0.04, cfg.norm)
+        ref = oracle.sign(cfg.dims, cfg.kappa, c["U"], coef, 0.04, cfg.norm, None, None, c["x"])
+        assert rel(to_host(op, op.apply_sign(dx)), ref) <= TOL_DOV
+
+
+def test_multishift_cg_vs_oracle(ovp, cfg0):
+    c = cfg0
+    cfg = c["cfg"]
+    op, coef = setup_op(ovp, c)
+    masses = (0.1, 0.005, 0.04)
+    x, iters, res, ok = op.multishift_cg(masses, to_dev(op, c["x"]), tol=1e-9, maxiter=300)
+    assert ok and np.all(res <= 1e-8)
+
+    def g5(v):
+        o = v.copy(); o[..., 2:, :] *= -1; return o
+    args = (cfg.dims, cfg.kappa, c["U"], coef, cfg.eps, cfg.norm, c["V"], c["lam"])
+    A = lambda v: g5(oracle.dov(*args, 0.0, g5(oracle.dov(*args, 0.0, v))))
+    xs, it_ref, res_ref = multishift_cg(A, [sigma_of_mass(m) for m in masses], c["x"], 1e-9, 300)
+    assert abs(iters - it_ref) <= 1
+    got = to_host(op, x)
+    for i in range(len(masses)):
+        assert rel(got[i], xs[i]) <= 1e-7  # two CG runs to tol 1e-9 each
+
+
+def test_lanczos_4x4_vs_dense(ovp, cfg0):
+    c = cfg0
+    cfg = c["cfg"]
+    op, _ = setup_op(ovp, c, with_small=False)
+    k = 8
+    V, lam, res, ok = op.lanczos_lowmodes(k, tol=1e-9, max_restarts=40, cheb_order=20, subspace=40)
+    assert ok and np.all(res <= 1e-9)
+    q = c["w"] / cfg.norm
+    exact = q[np.argsort(np.abs(q))[:k]]
+    assert np.max(np.abs(np.sort(lam) - np.sort(exact))) <= 1e-9
+    Vh = to_host(op, V)
+    for i in range(k):  # the oracle's own operator confirms each pair
+        r = oracle.hw(cfg.dims, cfg.kappa, c["U"], Vh[i]) / cfg.norm - lam[i] * Vh[i]
+        assert np.linalg.norm(r.ravel()) <= 1e-8
+    G = Vh.reshape(k, -1).conj() @ Vh.reshape(k, -1).T
+    assert np.max(np.abs(G - np.eye(k))) <= 1e-10
