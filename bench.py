@@ -1,0 +1,419 @@
+"""bench.py -- D_ov applies/s on the headline workload (BASELINE.json configs[3]: 24^3x64, fp64, n = 300,
+sqrt(eps) = 0.01, k = 100 low modes, 8 Gaussian sources), one process per GPU.
+
+A "step" is ONE pass of the whole hot path over one source: small-space projector (V^+x, x - Vc, V sgn c),
+the Clenshaw polynomial sign (2n+1 = 601 launches of the Wilson kernel with fused epilogues) and the D_ov
+assembly (fused into the last launch)  --  `ov_apply_dov` of include/ov.h.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W]          the CUDA library (this repo)
+  python bench.py --impl reference ...                          the CPU oracle on the host cores (reference arm)
+
+Multi-GPU: the path does not shard in this build (replicas only), so --gpus N runs N
+independent replicas (one per rank, each with its own sources) and reports the aggregate; no collective is on
+the data path.  Timing: CUDA events on the library's stream, barrier + synchronize on both sides, max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads as wl  # noqa: E402
+
+METRIC = "D_ov applies/sec"
+UNIT = "applies/s"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=8)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=["b200", "reference"], default="b200")
+    ap.add_argument("--config", type=int, default=3, help="index into BASELINE.json configs (3 = headline)")
+    ap.add_argument("--order", type=int, default=None, help="override the Chebyshev order (testing only)")
+    ap.add_argument("--k", type=int, default=None, help="override the number of low modes (testing only)")
+    ap.add_argument("--recon", type=int, default=18, choices=[18, 12])
+    ap.add_argument("--variant", type=int, default=0, help="dslash kernel variant (0 = automatic)")
+    ap.add_argument("--modes-file", default=None,
+                    help="torch file with the low modes {V, lam}: loaded if present, else written after Lanczos")
+    ap.add_argument("--lanczos-order", type=int, default=100, help="Chebyshev filter order (paper: 100)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+def workload_name(cfg, order, k):
+    return (f"configs[{cfg.index}] {cfg.name} fp64, links spread {cfg.spread}, kappa {cfg.kappa}, Chebyshev order "
+            f"{order}, sqrt(eps) {cfg.sqrt_eps}, k={k} low modes, {cfg.nsrc} Gaussian sources, one D_ov apply per step")
+
+
+# ---------------------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4): "sw_power_cap",
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop.wait(0.1)
+
+    def __enter__(self):
+        if self.nv is not None:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["nvml unavailable"]}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons)}
+
+
+# ---------------------------------------------------------------------------------------------- CPU oracle legs
+def stand_in_modes(dims, k, seed):
+    """k orthonormal stand-in vectors (Gaussian, vector i supported on the sites with index = i mod k) with
+    lambda = +-0.05: the oracle cannot compute low modes at this size (O9); for TIMING the projector
+    only its shape matters (the oracle loops over every element of every vector)."""
+    rng = np.random.default_rng(seed)
+    X, Y, Z, T = dims
+    nsite = wl.volume(dims)
+    V = np.zeros((k, nsite, 12), dtype=np.complex128)
+    for i in range(k):
+        m = len(range(i, nsite, k))
+        V[i, i::k] = rng.standard_normal((m, 12)) + 1j * rng.standard_normal((m, 12))
+        V[i] /= np.linalg.norm(V[i])
+    lam = 0.05 * np.where(np.arange(k) % 2 == 0, 1.0, -1.0)
+    return V.reshape(k, T, Z, Y, X, 4, 3), lam
+
+
+class OracleSample:
+    """The oracle, as it stands, on a bounded sample of the workload: the oracle's D_ov on the FULL lattice with a
+    reduced order n_s (2 n_s + 1 H_w applies instead of 2 n + 1) and k_s = ceil(k (2 n_s + 1)/(2 n + 1)) low modes,
+    its wall time scaled by (2 n + 1)/(2 n_s + 1) to one order-n apply."""
+
+    def __init__(self, cfg, order, k, U, budget_s, nsteps):
+        import oracle
+        from oracle import chebyshev as ch
+        self.oracle = oracle
+        self.cfg, self.order, self.k, self.U = cfg, order, k, U
+        self.x = wl.gaussian_source(cfg.dims, wl.source_seed(cfg.index, 0))
+        oracle.hw(cfg.dims, cfg.kappa, U, self.x)  # page in, spin up the OpenMP team
+        t0 = time.perf_counter()
+        oracle.hw(cfg.dims, cfg.kappa, U, self.x)
+        self.t_hw = time.perf_counter() - t0
+        per_step = budget_s / max(1, nsteps)
+        n_s = int(max(1, min(order, (per_step / max(self.t_hw, 1e-9) - 1) // 2)))
+        self.n_s = n_s
+        self.scale = (2 * order + 1) / (2 * n_s + 1)
+        self.k_s = int(min(k, max(1, round(k / self.scale)))) if k > 0 else 0
+        self.coef = ch.cheb_coeffs(n_s, cfg.eps)
+        self.V, self.lam = stand_in_modes(cfg.dims, self.k_s, 7) if self.k_s else (None, None)
+        self.cores = oracle.num_threads()
+
+    def step(self):
+        c = self.cfg
+        t0 = time.perf_counter()
+        self.oracle.dov(c.dims, c.kappa, self.U, self.coef, c.eps, c.norm, self.V, self.lam, 0.0, self.x)
+        return (time.perf_counter() - t0) * self.scale  # seconds per full-order apply
+
+    def describe(self):
+        return (f"oracle D_ov on the full {self.cfg.name} lattice at order {self.n_s} ({2 * self.n_s + 1} H_w applies) "
+                f"with {self.k_s} stand-in low modes; time x {self.scale:.2f} = one order-{self.order} apply with "
+                f"k={self.k}; oracle H_w alone: {wl.volume(self.cfg.dims) / self.t_hw / 1e6:.2f} Msites/s")
+
+
+def run_reference(args):
+    rank, world, _ = dist_env()
+    if rank != 0:
+        return 0
+    cfg = wl.CONFIGS[args.config]
+    order = args.order if args.order is not None else cfg.order
+    k = args.k if args.k is not None else cfg.k
+    U = wl.su3_links(cfg.dims, cfg.spread, wl.gauge_seed(cfg.index))
+    smp = OracleSample(cfg, order, k, U, budget_s=150.0, nsteps=args.steps + args.warmup)
+    for _ in range(args.warmup):
+        smp.step()
+    times = [smp.step() for _ in range(args.steps)]
+    sec = float(np.mean(times))
+    value = 1.0 / sec
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sec, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(cfg, order, k), "note": "CPU oracle on host cores; rank 0 only"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": smp.cores, "kind": "oracle", "sample": smp.describe()},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ---------------------------------------------------------------------------------------------- the CUDA arm
+def algorithmic_bytes_per_sign(order, V, with_low):
+    """Algorithmic HBM bytes of the 2n+1 Wilson launches of one polynomial sign: every
+    launch reads the spinor (192 B/site), the 4 links of the site (576) and writes 192; the second launch of each
+    Clenshaw order also reads x, b_{j+1}, b_{j+2} (the first order has no b_{j+2}); the last launch reads x and,
+    with a small space, x_low."""
+    base = 960
+    total = 0
+    for j in range(order - 1, -1, -1):
+        total += base                                   # t = Q b_{j+1}
+        total += base + 192 * (2 if j == order - 1 else 3)
+    total += base + 192 * (2 if with_low else 1)        # D_ov assembly in the final epilogue
+    return total * V
+
+
+def get_low_modes(op, cfg, k, args, log):
+    import torch
+    path = args.modes_file
+    if path and os.path.exists(path):
+        d = torch.load(path, map_location="cpu")
+        if d["V"].shape[0] >= k and tuple(d["dims"]) == tuple(cfg.dims):
+            log(f"low modes: loaded {path}")
+            return d["V"][:k].cuda().contiguous(), np.asarray(d["lam"][:k]), float(d["resid"]), 0.0
+    t0 = time.perf_counter()
+    V, lam, res, ok = op.lanczos_lowmodes(k, tol=1e-8, max_restarts=60, cheb_order=args.lanczos_order)
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    log(f"low modes: Lanczos k={k} in {dt:.1f} s, max residual {res.max():.2e}, converged={ok}, "
+        f"|lambda| in [{np.abs(lam).min():.5f}, {np.abs(lam).max():.5f}]")
+    if not ok:
+        raise RuntimeError(f"Lanczos did not reach 1e-8 (max residual {res.max():.2e})")
+    if path:
+        torch.save({"V": V.cpu(), "lam": lam, "resid": float(res.max()), "dims": tuple(cfg.dims)}, path)
+    return V, lam, float(res.max()), dt
+
+
+def run_b200(args):
+    import torch
+    import torch.distributed as dist
+    import paper_1111_6288_b200 as ovp
+    from paper_1111_6288_b200 import build as ovbuild
+
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (this library has no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        ovbuild.build()
+    if world > 1:
+        dist.barrier()
+    ovp.load_library()
+    log = (lambda m: print(f"[bench] {m}", file=sys.stderr, flush=True)) if rank == 0 else (lambda m: None)
+
+    cfg = wl.CONFIGS[args.config]
+    order = args.order if args.order is not None else cfg.order
+    k = args.k if args.k is not None else cfg.k
+    V_sites = wl.volume(cfg.dims)
+    t0 = time.perf_counter()
+    U = wl.su3_links(cfg.dims, cfg.spread, wl.gauge_seed(cfg.index))
+    log(f"links generated in {time.perf_counter() - t0:.1f} s")
+    op = ovp.Overlap(cfg.dims, cfg.kappa, U, recon=args.recon)
+    if args.variant:
+        op.set_dslash_variant(args.variant)
+    coef = ovp.chebyshev_coeffs(order, cfg.eps)
+    op.set_polynomial(coef, cfg.eps, cfg.norm)
+    lanczos_s, resid = 0.0, None
+    if k > 0:
+        Vlow, lam, resid, lanczos_s = get_low_modes(op, cfg, k, args, log)
+        op.set_smallspace(Vlow, lam)
+
+    # sources: rank r takes its own seeds (replicas work on independent sources)
+    nsrc = cfg.nsrc
+    host_src = [torch.from_numpy(wl.gaussian_source(cfg.dims, wl.source_seed(cfg.index, rank * nsrc + j))).pin_memory()
+                for j in range(nsrc)]
+    dev_src = [op.pack_spinor(h.cuda(non_blocking=True)) for h in host_src]
+    out = op.new_spinor()
+    host_out = torch.empty_like(host_src[0]).pin_memory()
+    torch.cuda.synchronize()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    def timed(fn, nwarm, nstep, sampler=None):
+        for i in range(nwarm):
+            fn(i)
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ctxm = sampler if sampler is not None else _Null()
+        with ctxm:
+            e0.record(op.stream)
+            for i in range(nstep):
+                fn(nwarm + i)
+            e1.record(op.stream)
+            barrier()
+        ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+        return float(ms.item())
+
+    # ---- device-resident: the headline value
+    sampler = ClockSampler(local)
+    torch.cuda.cudart().cudaProfilerStart()
+    op.timing_enable(False)
+    for i in range(args.warmup):
+        op.apply_dov(0.0, dev_src[i % nsrc], out)
+    op.timing_enable(True)
+    l0 = op.launch_count
+    ms = timed(lambda i: op.apply_dov(0.0, dev_src[i % nsrc], out), 0, args.steps, sampler)
+    launches = op.launch_count - l0
+    tim = op.timing_read()
+    op.timing_enable(False)
+    torch.cuda.cudart().cudaProfilerStop()
+    value = world * args.steps / (ms * 1e-3)
+
+    # ---- end to end through the host-buffer entry point (H2D + D2H inside the timed region)
+    e2e = None
+    if not args.no_e2e:
+        ne = max(2, min(args.steps, 4))
+        ms_e = timed(lambda i: op.apply_dov_host(0.0, host_src[i % nsrc], host_out), 1, ne)
+        nbytes = host_src[0].numel() * 16
+        e2e = {"value": world * ne / (ms_e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": nbytes,
+               "d2h_bytes_per_step": nbytes, "steps": ne}
+
+    # ---- the Wilson kernel alone (ping-pong, working set gauge + 2 spinors > L2), for the extra keys
+    a, b = dev_src[0].clone(), op.new_spinor()
+    nhw = 100
+    ms_hw = timed(lambda i: op.apply_hw(a, b) if i % 2 == 0 else op.apply_hw(b, a), 10, nhw)
+    del a, b
+    hw_gbs = 960.0 * V_sites * nhw / (ms_hw * 1e-3) / 1e9
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+    return finish(args, cfg, order, k, V_sites, world, ms, value, launches, tim, e2e, hw_gbs, ms_hw / nhw,
+                  sampler, lanczos_s, resid, U, log)
+
+
+class _Null:
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        return False
+
+
+def measured_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic():
+    """dram bytes per launch of the Wilson kernel from the committed `ncu --set full` capture, if any."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "wilson_traffic.json")) as f:
+            return json.load(f)
+    except Exception:
+        return None
+
+
+def finish(args, cfg, order, k, V_sites, world, ms, value, launches, tim, e2e, hw_gbs, hw_ms, sampler,
+           lanczos_s, resid, U, log):
+    peak, peak_src = measured_peak()
+    nsign = args.steps
+    wl_launches = tim["wilson_launches"]
+    alg_bytes = algorithmic_bytes_per_sign(order, V_sites, k > 0) * nsign / max(1, wl_launches)  # per launch
+    avg_ms = tim["wilson_ms"] / max(1, wl_launches)
+    achieved = alg_bytes / (avg_ms * 1e-3) / 1e9
+    tr = ncu_traffic()
+    roofline = {
+        "bound": "hbm", "kernel": "wilson_kernel (Wilson hopping term + fused gamma5/scale/Clenshaw-axpy epilogue)",
+        "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+        "traffic": (tr or {}).get("dram_bytes_per_launch"), "peak_source": peak_src,
+        "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_ms": avg_ms, "launches_timed": wl_launches,
+        "share_of_step": tim["wilson_ms"] / ms,
+        "projector": {"ms_per_step": tim["projector_ms"] / nsign,
+                      "GB/s": ((2 * k + 4) * 192.0 * V_sites) / max(1e-9, tim["projector_ms"] / nsign * 1e-3) / 1e9},
+        "hw_alone": {"GB/s": hw_gbs, "frac": hw_gbs / peak, "ms": hw_ms, "GFLOP/s": 1392.0 * V_sites / (hw_ms * 1e-3) / 1e9,
+                     "note": "100 back-to-back ov_apply_hw, ping-pong, 960 B/site"},
+    }
+    cpu = None
+    if not args.no_cpu_baseline and world == 1:
+        smp = OracleSample(cfg, order, k, U, budget_s=20.0, nsteps=1)
+        sec = smp.step()
+        cpu = {"value": 1.0 / sec, "unit": UNIT, "cores": smp.cores, "kind": "oracle", "sample": smp.describe()}
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(cfg, order, k), "recon": args.recon, "parallelism": f"replicas x{world}",
+                   "l2": "inputs larger than L2 (gauge 510 MB + 17 GB of low modes stream every step)",
+                   "low_modes": f"GPU Lanczos, max residual {resid:.1e}, {lanczos_s:.0f} s (untimed setup)" if k else "none"},
+        "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
+        "paper_context": "paper: ~30 CPU cores per GPU on unnamed 6 GB GPUs vs Cray XT-5 (PAPER.md:9) - context only",
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_b200(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -62,6 +62,12 @@ size_t ov_spinor_bytes(const ov_ctx* ctx); /* 192 * V */
 long long ov_volume(const ov_ctx* ctx);
 /* number of CUDA kernels this context has launched since creation (for bench.py's gpu_launches) */
 long long ov_launch_count(const ov_ctx* ctx);
+/* live timing for bench.py's roofline (CUDA events on the context's stream, recorded inside the calls that
+ * follow): ov_timing_enable(ctx, 1) starts accumulating, ov_timing_read synchronises and returns
+ * out_host[4] = { ms inside the Wilson/Clenshaw sweeps of ov_apply_sign/dov, kernel launches in them,
+ *                 ms inside the small-space projector, kernel launches in it }  and resets the accumulators. */
+int ov_timing_enable(ov_ctx* ctx, int on);
+int ov_timing_read(ov_ctx* ctx, double* out_host);
 /* selects the dslash kernel: 0 = automatic, 1 = gather (one thread per site, cache-reliant),
  * 2 = tiled (shared-memory staged).  Returns OV_EINVAL if the variant cannot run on this lattice. */
 int ov_set_dslash_variant(ov_ctx* ctx, int variant);

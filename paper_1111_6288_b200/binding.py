@@ -21,6 +21,7 @@ _CODES = {1: "OV_EINVAL", 2: "OV_ENOMEM", 3: "OV_ECUDA", 4: "OV_ESTATE", 5: "OV_
 # every symbol include/ov.h declares (tests check that the library exports all of them)
 SYMBOLS = [
     "ov_create", "ov_destroy", "ov_last_error", "ov_spinor_bytes", "ov_volume", "ov_launch_count",
+    "ov_timing_enable", "ov_timing_read",
     "ov_set_dslash_variant", "ov_pack_spinor", "ov_unpack_spinor", "ov_dslash", "ov_apply_hw",
     "ov_chebyshev_coeffs", "ov_set_polynomial", "ov_set_smallspace", "ov_project", "ov_apply_sign",
     "ov_apply_dov", "ov_apply_hw_host", "ov_apply_dov_host", "ov_blas_axpy", "ov_blas_scale", "ov_blas_dot",
@@ -140,6 +141,15 @@ class Overlap:
     @property
     def launch_count(self):
         return int(self.lib.ov_launch_count(self._ctx))
+
+    def timing_enable(self, on=True):
+        self._check(self.lib.ov_timing_enable(self._ctx, ctypes.c_int(1 if on else 0)))
+
+    def timing_read(self):
+        """{wilson_ms, wilson_launches, projector_ms, projector_launches} since the last read."""
+        out = (ctypes.c_double * 4)()
+        self._check(self.lib.ov_timing_read(self._ctx, out))
+        return dict(wilson_ms=out[0], wilson_launches=int(out[1]), projector_ms=out[2], projector_launches=int(out[3]))
 
     def set_dslash_variant(self, v):
         self._check(self.lib.ov_set_dslash_variant(self._ctx, ctypes.c_int(v)))

@@ -57,6 +57,27 @@ int launch_wilson(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& 
     return launch_wilson_gather(ctx, in, out, ep);
 }
 
+Span::Span(ov_ctx* c, int phase) : ctx(c) {
+    if (!c->timing) return;
+    if (2 * c->ev_used + 2 > c->ev_pool.size()) {
+        cudaEvent_t a, b;
+        if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return;
+        c->ev_pool.push_back(a);
+        c->ev_pool.push_back(b);
+        c->ev_phase.push_back(0);
+        c->ev_launches.push_back(0);
+    }
+    slot = (int)c->ev_used++;
+    c->ev_phase[slot] = phase;
+    launches0 = c->launches;
+    cudaEventRecord(c->ev_pool[2 * slot], c->stream);
+}
+Span::~Span() {
+    if (slot < 0) return;
+    cudaEventRecord(ctx->ev_pool[2 * slot + 1], ctx->stream);
+    ctx->ev_launches[slot] = ctx->launches - launches0;
+}
+
 static bool overlaps(const ov_ctx* ctx, const void* a, const void* b, int nrhs) {
     const char* pa = (const char*)a;
     const char* pb = (const char*)b;
@@ -116,6 +137,7 @@ void ov_destroy(ov_ctx* ctx) {
     cudaFree(ctx->host_stage_in);
     cudaFree(ctx->host_stage_abi);
     cudaFree(ctx->host_stage_out);
+    for (auto e : ctx->ev_pool) cudaEventDestroy(e);
     delete ctx;
 }
 
@@ -123,6 +145,31 @@ const char* ov_last_error(const ov_ctx* ctx) { return ctx ? ctx->err.c_str() : "
 size_t ov_spinor_bytes(const ov_ctx* ctx) { return ctx ? spinor_elems(ctx) * sizeof(double2) : 0; }
 long long ov_volume(const ov_ctx* ctx) { return ctx ? ctx->lat.V : 0; }
 long long ov_launch_count(const ov_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int ov_timing_enable(ov_ctx* ctx, int on) {
+    if (!ctx) return OV_EINVAL;
+    OV_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    ctx->timing = on != 0;
+    ctx->ev_used = 0;
+    return OV_OK;
+}
+
+int ov_timing_read(ov_ctx* ctx, double* out_host) {
+    if (!ctx) return OV_EINVAL;
+    if (!out_host) return fail(ctx, OV_EINVAL, "null pointer");
+    OV_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    double ms[2] = {0, 0}, launches[2] = {0, 0};
+    for (size_t i = 0; i < ctx->ev_used; i++) {
+        float t = 0.f;
+        OV_CUDA(ctx, cudaEventElapsedTime(&t, ctx->ev_pool[2 * i], ctx->ev_pool[2 * i + 1]));
+        ms[ctx->ev_phase[i]] += t;
+        launches[ctx->ev_phase[i]] += (double)ctx->ev_launches[i];
+    }
+    out_host[0] = ms[0]; out_host[1] = launches[0];
+    out_host[2] = ms[1]; out_host[3] = launches[1];
+    ctx->ev_used = 0;
+    return OV_OK;
+}
 
 int ov_set_dslash_variant(ov_ctx* ctx, int variant) {
     if (!ctx) return OV_EINVAL;

@@ -67,6 +67,13 @@ struct ov_ctx {
     double2* host_stage_in = nullptr;   // device staging for *_host calls (canonical)
     double2* host_stage_abi = nullptr;
     double2* host_stage_out = nullptr;
+
+    // live timing (ov_timing_enable): CUDA-event pairs on ctx->stream around the two phases of an apply
+    bool timing = false;
+    std::vector<cudaEvent_t> ev_pool;   // recorded pairs: [2i] start, [2i+1] stop
+    std::vector<int> ev_phase;          // phase of pair i: 0 = Wilson/Clenshaw sweep, 1 = projector
+    std::vector<long long> ev_launches; // kernel launches inside pair i
+    size_t ev_used = 0;                 // pairs in use
 };
 
 namespace ov {
@@ -126,6 +133,15 @@ int launch_multi_axpy(ov_ctx* ctx, const double2* xs, size_t stride, int nvec, i
 
 // projector: c = V^+ x (left in ctx->d_result[0..k)); perp = x - V c; low = V (sgn o c)
 int project(ov_ctx* ctx, const double2* x, double2* perp, double2* low);
+
+// live timing: a Span records an event pair on ctx->stream around a phase when ctx->timing is on
+struct Span {
+    ov_ctx* ctx;
+    int slot = -1;
+    long long launches0 = 0;
+    Span(ov_ctx* c, int phase);
+    ~Span();
+};
 
 // operator drivers
 int sign_poly(ov_ctx* ctx, const double2* x, double2* out, const Epilogue& fin);

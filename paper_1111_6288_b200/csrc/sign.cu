@@ -25,6 +25,7 @@ __global__ void projector_coef_kernel(const double2* __restrict__ c, const doubl
 // all of the H_w eigenvectors for each matrix multiplication"): 2 k 192 B/site + 4 spinors.
 int project(ov_ctx* ctx, const double2* x, double2* perp, double2* low) {
     const size_t stride = spinor_elems(ctx);
+    Span span(ctx, 1);
     OV_TRY(launch_multi_dot(ctx, ctx->Vlow, stride, ctx->k, x));
     projector_coef_kernel<<<(ctx->k + 127) / 128, 128, 0, ctx->stream>>>(ctx->d_result, ctx->d_sgn, ctx->k, ctx->d_coef);
     ctx->launches++;
@@ -49,13 +50,13 @@ int sign_poly(ov_ctx* ctx, const double2* x, double2* out, const Epilogue& fin) 
     OV_TRY(workspace(ctx, 1, &b2));
     OV_TRY(workspace(ctx, 2, &t));
 
+    // b_n = c_n x  (b_{n+1} = b_{n+2} = 0)
+    OV_TRY(launch_axpby(ctx, c[n], x, 0.0, nullptr, b1));
+    Span span(ctx, 0);  // from here on every launch is the Wilson kernel
     const double2* y = nullptr;
     if (n == 0) {
-        OV_TRY(launch_axpby(ctx, c[0], x, 0.0, nullptr, b1));
         y = b1;
     } else {
-        // b_n = c_n x  (b_{n+1} = b_{n+2} = 0)
-        OV_TRY(launch_axpby(ctx, c[n], x, 0.0, nullptr, b1));
         bool b2_valid = false;
         for (int j = n - 1; j >= 0; j--) {
             Epilogue e1;  // t = Q b1
