@@ -201,13 +201,34 @@ def run_reference(args):
     return 0
 
 
+# ---------------------------------------------------------------------------------------------- replicas (N > 1)
+def replica_source_seeds(cfg, rank):
+    """Replicas work on independent sources: rank r takes source indices r*nsrc .. (r+1)*nsrc - 1."""
+    return [wl.source_seed(cfg.index, rank * cfg.nsrc + j) for j in range(cfg.nsrc)]
+
+
+def max_over_ranks(ms, world, device):
+    """The job's time is the slowest replica's (device-timed) time."""
+    import torch
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(world, steps, ms):
+    """Whole-job throughput: every one of the `world` replicas did `steps` applies in `ms` (max over ranks)."""
+    return world * steps / (ms * 1e-3)
+
+
 # ---------------------------------------------------------------------------------------------- the CUDA arm
-def algorithmic_bytes_per_sign(order, V, with_low):
+def algorithmic_bytes_per_sign(order, V, with_low, recon=18):
     """Algorithmic HBM bytes of the 2n+1 Wilson launches of one polynomial sign: every
     launch reads the spinor (192 B/site), the 4 links of the site (576) and writes 192; the second launch of each
     Clenshaw order also reads x, b_{j+1}, b_{j+2} (the first order has no b_{j+2}); the last launch reads x and,
     with a small space, x_low."""
-    base = 960
+    base = 192 + 4 * (recon // 2) * 16 + 192   # 960 (recon 18) / 768 (recon 12)
     total = 0
     for j in range(order - 1, -1, -1):
         total += base                                   # t = Q b_{j+1}
@@ -220,10 +241,10 @@ def get_low_modes(op, cfg, k, args, log):
     import torch
     path = args.modes_file
     if path and os.path.exists(path):
-        d = torch.load(path, map_location="cpu")
-        if d["V"].shape[0] >= k and tuple(d["dims"]) == tuple(cfg.dims):
+        d = torch.load(path, map_location="cpu", weights_only=True)
+        if d["V"].shape[0] >= k and tuple(d["dims"].tolist()) == tuple(cfg.dims):
             log(f"low modes: loaded {path}")
-            return d["V"][:k].cuda().contiguous(), np.asarray(d["lam"][:k]), float(d["resid"]), 0.0
+            return d["V"][:k].cuda().contiguous(), d["lam"][:k].numpy(), float(d["resid"]), 0.0
     t0 = time.perf_counter()
     V, lam, res, ok = op.lanczos_lowmodes(k, tol=1e-8, max_restarts=60, cheb_order=args.lanczos_order)
     torch.cuda.synchronize()
@@ -233,7 +254,8 @@ def get_low_modes(op, cfg, k, args, log):
     if not ok:
         raise RuntimeError(f"Lanczos did not reach 1e-8 (max residual {res.max():.2e})")
     if path:
-        torch.save({"V": V.cpu(), "lam": lam, "resid": float(res.max()), "dims": tuple(cfg.dims)}, path)
+        torch.save({"V": V.cpu(), "lam": torch.from_numpy(lam), "resid": torch.tensor(float(res.max())),
+                    "dims": torch.tensor(cfg.dims)}, path)
     return V, lam, float(res.max()), dt
 
 
@@ -275,8 +297,8 @@ def run_b200(args):
 
     # sources: rank r takes its own seeds (replicas work on independent sources)
     nsrc = cfg.nsrc
-    host_src = [torch.from_numpy(wl.gaussian_source(cfg.dims, wl.source_seed(cfg.index, rank * nsrc + j))).pin_memory()
-                for j in range(nsrc)]
+    host_src = [torch.from_numpy(wl.gaussian_source(cfg.dims, sd)).pin_memory()
+                for sd in replica_source_seeds(cfg, rank)]
     dev_src = [op.pack_spinor(h.cuda(non_blocking=True)) for h in host_src]
     out = op.new_spinor()
     host_out = torch.empty_like(host_src[0]).pin_memory()
@@ -300,10 +322,7 @@ def run_b200(args):
                 fn(nwarm + i)
             e1.record(op.stream)
             barrier()
-        ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(ms, op=dist.ReduceOp.MAX)
-        return float(ms.item())
+        return max_over_ranks(e0.elapsed_time(e1), world, "cuda")
 
     # ---- device-resident: the headline value
     sampler = ClockSampler(local)
@@ -318,7 +337,7 @@ def run_b200(args):
     tim = op.timing_read()
     op.timing_enable(False)
     torch.cuda.cudart().cudaProfilerStop()
-    value = world * args.steps / (ms * 1e-3)
+    value = aggregate_value(world, args.steps, ms)
 
     # ---- end to end through the host-buffer entry point (H2D + D2H inside the timed region)
     e2e = None
@@ -326,7 +345,7 @@ def run_b200(args):
         ne = max(2, min(args.steps, 4))
         ms_e = timed(lambda i: op.apply_dov_host(0.0, host_src[i % nsrc], host_out), 1, ne)
         nbytes = host_src[0].numel() * 16
-        e2e = {"value": world * ne / (ms_e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": nbytes,
+        e2e = {"value": aggregate_value(world, ne, ms_e), "unit": UNIT, "h2d_bytes_per_step": nbytes,
                "d2h_bytes_per_step": nbytes, "steps": ne}
 
     # ---- the Wilson kernel alone (ping-pong, working set gauge + 2 spinors > L2), for the extra keys
@@ -334,7 +353,7 @@ def run_b200(args):
     nhw = 100
     ms_hw = timed(lambda i: op.apply_hw(a, b) if i % 2 == 0 else op.apply_hw(b, a), 10, nhw)
     del a, b
-    hw_gbs = 960.0 * V_sites * nhw / (ms_hw * 1e-3) / 1e9
+    hw_gbs = (384.0 + 32.0 * args.recon) * V_sites * nhw / (ms_hw * 1e-3) / 1e9
 
     if rank != 0:
         if world > 1:
@@ -374,7 +393,7 @@ def finish(args, cfg, order, k, V_sites, world, ms, value, launches, tim, e2e, h
     peak, peak_src = measured_peak()
     nsign = args.steps
     wl_launches = tim["wilson_launches"]
-    alg_bytes = algorithmic_bytes_per_sign(order, V_sites, k > 0) * nsign / max(1, wl_launches)  # per launch
+    alg_bytes = algorithmic_bytes_per_sign(order, V_sites, k > 0, args.recon) * nsign / max(1, wl_launches)  # per launch
     avg_ms = tim["wilson_ms"] / max(1, wl_launches)
     achieved = alg_bytes / (avg_ms * 1e-3) / 1e9
     tr = ncu_traffic()
@@ -387,7 +406,7 @@ def finish(args, cfg, order, k, V_sites, world, ms, value, launches, tim, e2e, h
         "projector": {"ms_per_step": tim["projector_ms"] / nsign,
                       "GB/s": ((2 * k + 4) * 192.0 * V_sites) / max(1e-9, tim["projector_ms"] / nsign * 1e-3) / 1e9},
         "hw_alone": {"GB/s": hw_gbs, "frac": hw_gbs / peak, "ms": hw_ms, "GFLOP/s": 1392.0 * V_sites / (hw_ms * 1e-3) / 1e9,
-                     "note": "100 back-to-back ov_apply_hw, ping-pong, 960 B/site"},
+                     "note": f"100 back-to-back ov_apply_hw, ping-pong, {384 + 32 * args.recon} B/site"},
     }
     cpu = None
     if not args.no_cpu_baseline and world == 1:

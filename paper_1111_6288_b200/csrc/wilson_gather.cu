@@ -23,6 +23,13 @@ struct GatherArgs {
     Epilogue ep;
 };
 
+// 64-thread blocks at <= 168 registers: 6 blocks = 12 warps per SM.  Measured at 24^3x64 (profiles/): 128 threads with
+// no register cap ran at 8 warps/SM and 215 us per apply, this shape at 166 us.
+constexpr int kGatherThreads = 64;
+constexpr int kGatherMinBlocks = 6;
+
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
 template <int RECON>
 __device__ __forceinline__ void load_link(const double2* __restrict__ gauge, long long V, int mu,
                                           long long site, double2* __restrict__ u) {
@@ -45,8 +52,9 @@ __device__ __forceinline__ void hop(double2* __restrict__ acc, const GatherArgs&
     reconstruct_add<MU, SIGMA>(acc, g, ph);
 }
 
-template <int RECON>
-__global__ void __launch_bounds__(128) wilson_gather_kernel(const GatherArgs a) {
+// NA: number of epilogue operands A1..A_NA (always filled in order); NA = -1: hop only
+template <int RECON, int NA>
+__global__ void __launch_bounds__(kGatherThreads, kGatherMinBlocks) wilson_gather_kernel(const GatherArgs a) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= a.V) return;
     long long r = i;
@@ -55,6 +63,14 @@ __global__ void __launch_bounds__(128) wilson_gather_kernel(const GatherArgs a) 
     const int z = (int)(r % a.Z);
     const int t = (int)(r / a.Z);
     const long long sX = 1, sY = a.X, sZ = (long long)a.X * a.Y, sT = (long long)a.X * a.Y * a.Z;
+
+    // the epilogue operands are read only after the whole stencil: pull them into L2 now so those late loads hit
+#pragma unroll
+    for (int c = 0; c < 12; c++) {
+        if (NA >= 1) prefetch_l2(a.ep.A1 + (long long)c * a.V + i);
+        if (NA >= 2) prefetch_l2(a.ep.A2 + (long long)c * a.V + i);
+        if (NA >= 3) prefetch_l2(a.ep.A3 + (long long)c * a.V + i);
+    }
 
     double2 acc[12];
 #pragma unroll
@@ -87,22 +103,38 @@ __global__ void __launch_bounds__(128) wilson_gather_kernel(const GatherArgs a) 
     }
 
     const Epilogue& ep = a.ep;
-    if (ep.hop_only) {
+    if (NA < 0) {
 #pragma unroll
         for (int c = 0; c < 12; c++) a.out[(long long)c * a.V + i] = acc[c];
         return;
     }
     const double slo = ep.g5 ? -ep.s : ep.s;
+    // `out` may alias an operand (the Clenshaw step writes b_j over b_{j+2}), so the compiler must keep every operand
+    // load behind the previous store: done component by component that is 12 dependent memory round trips.  Load a
+    // chunk of components of every operand first (all loads in flight at once), then combine and store the chunk.
+    constexpr int CH = 4;
 #pragma unroll
-    for (int c = 0; c < 12; c++) {
-        const double sc = (c < 6) ? ep.s : slo;
-        const double2 own = __ldg(a.in + (long long)c * a.V + i);
-        double2 v = make_double2(sc * fma(-a.kappa, acc[c].x, own.x), sc * fma(-a.kappa, acc[c].y, own.y));
-        const bool lo = (c >= 6);
-        if (ep.A1) { const double2 w = ep.A1[(long long)c * a.V + i]; const double f = (lo && (ep.a_g5 & 1)) ? -ep.a1 : ep.a1; v.x = fma(f, w.x, v.x); v.y = fma(f, w.y, v.y); }
-        if (ep.A2) { const double2 w = ep.A2[(long long)c * a.V + i]; const double f = (lo && (ep.a_g5 & 2)) ? -ep.a2 : ep.a2; v.x = fma(f, w.x, v.x); v.y = fma(f, w.y, v.y); }
-        if (ep.A3) { const double2 w = ep.A3[(long long)c * a.V + i]; const double f = (lo && (ep.a_g5 & 4)) ? -ep.a3 : ep.a3; v.x = fma(f, w.x, v.x); v.y = fma(f, w.y, v.y); }
-        a.out[(long long)c * a.V + i] = v;
+    for (int c0 = 0; c0 < 12; c0 += CH) {
+        double2 own[CH], w1[CH], w2[CH], w3[CH];
+#pragma unroll
+        for (int k = 0; k < CH; k++) {
+            const long long e = (long long)(c0 + k) * a.V + i;
+            own[k] = __ldg(a.in + e);
+            if (NA >= 1) w1[k] = ep.A1[e];
+            if (NA >= 2) w2[k] = ep.A2[e];
+            if (NA >= 3) w3[k] = ep.A3[e];
+        }
+#pragma unroll
+        for (int k = 0; k < CH; k++) {
+            const int c = c0 + k;
+            const bool lo = (c >= 6);
+            const double sc = lo ? slo : ep.s;
+            double2 v = make_double2(sc * fma(-a.kappa, acc[c].x, own[k].x), sc * fma(-a.kappa, acc[c].y, own[k].y));
+            if (NA >= 1) { const double f = (lo && (ep.a_g5 & 1)) ? -ep.a1 : ep.a1; v.x = fma(f, w1[k].x, v.x); v.y = fma(f, w1[k].y, v.y); }
+            if (NA >= 2) { const double f = (lo && (ep.a_g5 & 2)) ? -ep.a2 : ep.a2; v.x = fma(f, w2[k].x, v.x); v.y = fma(f, w2[k].y, v.y); }
+            if (NA >= 3) { const double f = (lo && (ep.a_g5 & 4)) ? -ep.a3 : ep.a3; v.x = fma(f, w3[k].x, v.x); v.y = fma(f, w3[k].y, v.y); }
+            a.out[(long long)c * a.V + i] = v;
+        }
     }
 }
 
@@ -115,12 +147,22 @@ int launch_wilson_gather(ov_ctx* ctx, const double2* in, double2* out, const Epi
     a.V = ctx->lat.V;
     a.kappa = ctx->kappa;
     a.ep = ep;
-    const int threads = 128;
+    const int threads = kGatherThreads;
     const unsigned blocks = (unsigned)((a.V + threads - 1) / threads);
-    if (ctx->recon == 12)
-        wilson_gather_kernel<12><<<blocks, threads, 0, ctx->stream>>>(a);
-    else
-        wilson_gather_kernel<18><<<blocks, threads, 0, ctx->stream>>>(a);
+    const int na = ep.hop_only ? -1 : (ep.A3 ? 3 : ep.A2 ? 2 : ep.A1 ? 1 : 0);
+    if ((ep.A3 && !ep.A2) || (ep.A2 && !ep.A1)) return fail(ctx, OV_EINVAL, "epilogue operands must be filled in order");
+#define OV_GATHER(R, N) wilson_gather_kernel<R, N><<<blocks, threads, 0, ctx->stream>>>(a)
+#define OV_GATHER_NA(R)                                 \
+    switch (na) {                                       \
+        case -1: OV_GATHER(R, -1); break;               \
+        case 0: OV_GATHER(R, 0); break;                 \
+        case 1: OV_GATHER(R, 1); break;                 \
+        case 2: OV_GATHER(R, 2); break;                 \
+        default: OV_GATHER(R, 3); break;                \
+    }
+    if (ctx->recon == 12) { OV_GATHER_NA(12) } else { OV_GATHER_NA(18) }
+#undef OV_GATHER_NA
+#undef OV_GATHER
     ctx->launches++;
     OV_CUDA(ctx, cudaGetLastError());
     return OV_OK;
