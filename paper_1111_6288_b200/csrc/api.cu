@@ -113,7 +113,7 @@ int ov_create(ov_ctx** out, const int dims[4], double kappa, const void* gauge_d
     ctx->kappa = kappa;
     ctx->recon = recon;
     ctx->stream = (cudaStream_t)cuda_stream;
-    const size_t gbytes = (size_t)4 * (recon / 2) * ctx->lat.V * sizeof(double2);
+    const size_t gbytes = gauge_elems(ctx->lat.V, recon) * sizeof(double2);
     cudaError_t e = cudaMalloc(&ctx->gauge, gbytes);
     if (e != cudaSuccess) { delete ctx; return e == cudaErrorMemoryAllocation ? OV_ENOMEM : OV_ECUDA; }
     int rc = launch_gauge_relayout(ctx, (const double2*)gauge_dev);

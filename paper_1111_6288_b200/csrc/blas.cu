@@ -9,7 +9,7 @@
 namespace ov {
 
 // ------------------------------------------------------------------------------------------ layout
-// canonical gauge [site][mu][9] -> internal [mu][NE][site]
+// canonical gauge [site][mu][9] -> internal layout (gauge_index, ov_internal.h)
 template <int NE>
 __global__ void gauge_relayout_kernel(const double2* __restrict__ can, double2* __restrict__ g, long long V) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -17,7 +17,7 @@ __global__ void gauge_relayout_kernel(const double2* __restrict__ can, double2* 
 #pragma unroll
     for (int mu = 0; mu < 4; mu++)
 #pragma unroll
-        for (int e = 0; e < NE; e++) g[((long long)mu * NE + e) * V + i] = can[(i * 4 + mu) * 9 + e];
+        for (int e = 0; e < NE; e++) g[gauge_index<NE>(V, mu, e, i)] = can[(i * 4 + mu) * 9 + e];
 }
 
 int launch_gauge_relayout(ov_ctx* ctx, const double2* canonical) {

@@ -13,6 +13,22 @@ namespace ov {
 
 constexpr int kSpinorComplex = 12;  // 4 spins x 3 colours
 
+// Internal gauge layout.  Default: planes [mu][e][V] double2.  -DOV_GAUGE_BLOCKED selects [V/32][mu][e][32 sites] (the
+// 4 links of a warp's 32 consecutive sites contiguous in HBM); it measured +3% on a cold burst of the Wilson kernel at
+// 24^3x64 but nothing in the power-capped steady state of a D_ov apply, so the simpler layout stays.
+#ifdef OV_GAUGE_BLOCKED
+constexpr bool kGaugeBlocked = true;
+#else
+constexpr bool kGaugeBlocked = false;
+#endif
+// double2 index of entry e (0..NE-1) of link mu at `site`
+template <int NE>
+__host__ __device__ __forceinline__ long long gauge_index(long long V, int mu, int e, long long site) {
+    if (kGaugeBlocked) return (((site >> 5) * (4 * NE)) + (mu * NE + e)) * 32 + (site & 31);
+    return ((long long)(mu * NE + e)) * V + site;
+}
+inline size_t gauge_elems(long long V, int recon) { return (size_t)4 * (recon / 2) * (size_t)((V + 31) / 32 * 32); }
+
 struct Lattice {
     int X, Y, Z, T;
     long long V;  // sites
@@ -39,8 +55,9 @@ struct ov_ctx {
     double kappa = 0.0;
     int recon = 18;
     cudaStream_t stream = nullptr;
-    double2* gauge = nullptr;  // [mu][recon/2][V] double2
+    double2* gauge = nullptr;  // see gauge_index()
     int dslash_variant = 0;
+    int flip = 0;  // block order of the next Wilson launch (alternates)
     long long launches = 0;
     mutable std::string err;
 

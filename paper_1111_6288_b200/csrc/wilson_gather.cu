@@ -6,8 +6,10 @@
 //   hop(in)(x) = sum_mu [ s+ (1-gamma_mu) U_mu(x) in(x+mu) + s- (1+gamma_mu) U_mu(x-mu)^+ in(x-mu) ]
 //
 // Layouts: spinor component c of site i at double2 index c*V + i; link entry e (row-major) of U_mu(i) at
-// ((mu*NE)+e)*V + i with NE = 9 (recon 18) or 6 (recon 12).  A warp therefore reads 32 consecutive
-// double2 (512 B) per component: fully coalesced LDG.128.
+// gauge_index<NE>(V, mu, e, i) (ov_internal.h), NE = 9 (recon 18) or 6 (recon 12).  A warp reads 32 consecutive
+// double2 (512 B) per component or link entry: fully coalesced LDG.128.
+// Successive launches walk the lattice in opposite block order (GatherArgs::reverse): the spinor one launch wrote last
+// is what the next launch reads first, while it is still in the 126 MB L2.
 #include "ov_internal.h"
 #include "wilson_math.cuh"
 
@@ -20,6 +22,7 @@ struct GatherArgs {
     int X, Y, Z, T;
     long long V;
     double kappa;
+    int reverse;
     Epilogue ep;
 };
 
@@ -34,9 +37,10 @@ template <int RECON>
 __device__ __forceinline__ void load_link(const double2* __restrict__ gauge, long long V, int mu,
                                           long long site, double2* __restrict__ u) {
     constexpr int NE = RECON / 2;
-    const double2* p = gauge + ((long long)mu * NE) * V + site;
+    const double2* p = gauge + gauge_index<NE>(V, mu, 0, site);
+    const long long es = kGaugeBlocked ? 32 : V;  // stride between entries
 #pragma unroll
-    for (int e = 0; e < NE; e++) u[e] = __ldg(p + (long long)e * V);
+    for (int e = 0; e < NE; e++) u[e] = __ldg(p + (long long)e * es);
     if (RECON == 12) su3_row2(u);
 }
 
@@ -55,7 +59,8 @@ __device__ __forceinline__ void hop(double2* __restrict__ acc, const GatherArgs&
 // NA: number of epilogue operands A1..A_NA (always filled in order); NA = -1: hop only
 template <int RECON, int NA>
 __global__ void __launch_bounds__(kGatherThreads, kGatherMinBlocks) wilson_gather_kernel(const GatherArgs a) {
-    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const unsigned blk = a.reverse ? gridDim.x - 1 - blockIdx.x : blockIdx.x;
+    const long long i = (long long)blk * blockDim.x + threadIdx.x;
     if (i >= a.V) return;
     long long r = i;
     const int x = (int)(r % a.X); r /= a.X;
@@ -147,6 +152,12 @@ int launch_wilson_gather(ov_ctx* ctx, const double2* in, double2* out, const Epi
     a.V = ctx->lat.V;
     a.kappa = ctx->kappa;
     a.ep = ep;
+#ifdef OV_NO_ALTERNATE
+    a.reverse = 0;
+#else
+    a.reverse = ctx->flip;
+    ctx->flip ^= 1;
+#endif
     const int threads = kGatherThreads;
     const unsigned blocks = (unsigned)((a.V + threads - 1) / threads);
     const int na = ep.hop_only ? -1 : (ep.A3 ? 3 : ep.A2 ? 2 : ep.A1 ? 1 : 0);
