@@ -31,8 +31,6 @@ struct GatherArgs {
 constexpr int kGatherThreads = 64;
 constexpr int kGatherMinBlocks = 6;
 
-__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
-
 template <int RECON>
 __device__ __forceinline__ void load_link(const double2* __restrict__ gauge, long long V, int mu,
                                           long long site, double2* __restrict__ u) {
@@ -69,13 +67,6 @@ __global__ void __launch_bounds__(kGatherThreads, kGatherMinBlocks) wilson_gathe
     const int t = (int)(r / a.Z);
     const long long sX = 1, sY = a.X, sZ = (long long)a.X * a.Y, sT = (long long)a.X * a.Y * a.Z;
 
-    // the epilogue operands are read only after the whole stencil: pull them into L2 now so those late loads hit
-#pragma unroll
-    for (int c = 0; c < 12; c++) {
-        if (NA >= 1) prefetch_l2(a.ep.A1 + (long long)c * a.V + i);
-        if (NA >= 2) prefetch_l2(a.ep.A2 + (long long)c * a.V + i);
-        if (NA >= 3) prefetch_l2(a.ep.A3 + (long long)c * a.V + i);
-    }
 
     double2 acc[12];
 #pragma unroll
