@@ -130,8 +130,11 @@ int ov_blas_norm2(ov_ctx* ctx, const void* x, double* out_host);
  *   by Chebyshev-filtered thick-restart Lanczos on Q^2 followed by Rayleigh-Ritz in Q.  Needs the norm
  *   from ov_set_polynomial.  V_out_dev: k ABI spinors; lambda_out_host, resid_out_host: k values,
  *   resid_i = |Q v_i - lambda_i v_i|.  Returns OV_ENOCONV if some resid_i > tol after max_restarts.
- *   subspace = Krylov dimension m (0 = default 2k+16; the paper uses 2.5 k); cheb_order = degree of the
- *   filter in Q^2 (paper: 100).                                                                        */
+ *   subspace = Krylov dimension m (0 = default: 2k+16, reduced to what fits in free device memory; the paper uses
+ *   2.5 k); cheb_order = degree of the filter in Q^2 (paper: 100).
+ *   Memory: V_out_dev itself holds the first k basis vectors during the call (its contents are scratch until the
+ *   call returns); the library allocates the other m+1-k basis vectors + 3 spinors and frees them before returning.
+ *   All basis rotations are done in place, so k = 200 on 32^3x64 (80.5 GB of V) fits in 180 GB.                    */
 int ov_multishift_cg(ov_ctx* ctx, const double* masses_host, int nmass, const void* b, void* x, double tol,
                      int maxiter, int* iters_out, double* relres_out);
 int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_restarts, int cheb_order, int subspace,

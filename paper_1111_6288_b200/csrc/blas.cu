@@ -212,16 +212,22 @@ __global__ void __launch_bounds__(kRedThreads) reduce_partials_kernel(const doub
     if (threadIdx.x == 0) result[blockIdx.x] = sh[0];
 }
 
-int launch_multi_dot(ov_ctx* ctx, const double2* xs, size_t stride, int nvec, const double2* y) {
+int launch_multi_dot_at(ov_ctx* ctx, const double2* xs, size_t stride, int nvec, const double2* y, int result_offset,
+                        int result_total) {
     const long long n = (long long)spinor_elems(ctx);
     const long long nwarps = (n + kDotWarpElems - 1) / kDotWarpElems;
-    OV_TRY(ensure_reduction_buffers(ctx, (size_t)nwarps * nvec, (size_t)nvec));
+    OV_TRY(ensure_reduction_buffers(ctx, (size_t)nwarps * result_total, (size_t)result_total));
     const unsigned blocks = (unsigned)((nwarps + kDotThreads / 32 - 1) / (kDotThreads / 32));
-    multi_dot_kernel<<<blocks, kDotThreads, 0, ctx->stream>>>(xs, stride, nvec, y, n, nwarps, ctx->d_partial);
-    reduce_partials_kernel<<<nvec, kRedThreads, 0, ctx->stream>>>(ctx->d_partial, nwarps, ctx->d_result);
+    double2* partial = ctx->d_partial + (size_t)result_offset * nwarps;
+    multi_dot_kernel<<<blocks, kDotThreads, 0, ctx->stream>>>(xs, stride, nvec, y, n, nwarps, partial);
+    reduce_partials_kernel<<<nvec, kRedThreads, 0, ctx->stream>>>(partial, nwarps, ctx->d_result + result_offset);
     ctx->launches += 2;
     OV_CUDA(ctx, cudaGetLastError());
     return OV_OK;
+}
+
+int launch_multi_dot(ov_ctx* ctx, const double2* xs, size_t stride, int nvec, const double2* y) {
+    return launch_multi_dot_at(ctx, xs, stride, nvec, y, 0, nvec);
 }
 
 int fetch_results(ov_ctx* ctx, int n, double2* host_out) {
@@ -304,6 +310,59 @@ int launch_multi_axpy(ov_ctx* ctx, const double2* xs, size_t stride, int nvec, i
             return fail(ctx, OV_EINVAL, "multi_axpy: J must be 1, 2, 4 or 8");
     }
 #undef OV_MA_CASE
+    ctx->launches++;
+    OV_CUDA(ctx, cudaGetLastError());
+    return OV_OK;
+}
+
+}  // namespace ov
+
+namespace ov {
+
+// ------------------------------------------------------------------------------------------ in-place basis rotation
+// W[j] <- sum_{i<m} S[i][j] W[i]  for j < ncol <= m, in place (row a8: the restart and Rayleigh-Ritz rotations of the
+// Lanczos basis; at k = 200 on 32^3x64 a second copy of the basis would not fit in HBM).  The basis is two segments:
+// vectors 0..na-1 at a + i*stride, vectors na.. at b + (i-na)*stride.  A block stages a tile of kRotE elements of all
+// m vectors in shared memory, so every output can overwrite its input.  St is S transposed: St[j*m + i] (device).
+constexpr int kRotE = (int)(kRotTileBytesPerVector / sizeof(double2));
+constexpr int kRotThreads = 256;
+__global__ void __launch_bounds__(kRotThreads) rotate_inplace_kernel(double2* a, int na, double2* b, size_t stride, int m,
+                                                                     int ncol, const double2* __restrict__ St, long long n) {
+    extern __shared__ double2 tile[];  // [m][kRotE]
+    const long long e0 = (long long)blockIdx.x * kRotE;
+    const int el = threadIdx.x % kRotE, grp = threadIdx.x / kRotE;
+    constexpr int ngrp = kRotThreads / kRotE;
+    const bool live = e0 + el < n;
+    for (int i = grp; i < m; i += ngrp) {
+        const double2* v = (i < na) ? a + (size_t)i * stride : b + (size_t)(i - na) * stride;
+        tile[i * kRotE + el] = live ? v[e0 + el] : make_double2(0.0, 0.0);
+    }
+    __syncthreads();
+    for (int j = grp; j < ncol; j += ngrp) {
+        const double2* s = St + (size_t)j * m;
+        double2 acc0 = make_double2(0.0, 0.0), acc1 = make_double2(0.0, 0.0);
+        int i = 0;
+        for (; i + 2 <= m; i += 2) {
+            cmadd(acc0, __ldg(s + i), tile[i * kRotE + el]);
+            cmadd(acc1, __ldg(s + i + 1), tile[(i + 1) * kRotE + el]);
+        }
+        if (i < m) cmadd(acc0, __ldg(s + i), tile[i * kRotE + el]);
+        if (live) {
+            double2* v = (j < na) ? a + (size_t)j * stride : b + (size_t)(j - na) * stride;
+            v[e0 + el] = cadd(acc0, acc1);
+        }
+    }
+}
+
+int launch_rotate_inplace(ov_ctx* ctx, double2* a, int na, double2* b, size_t stride, int m, int ncol,
+                          const double2* St_dev) {
+    const long long n = (long long)spinor_elems(ctx);
+    const size_t shmem = (size_t)m * kRotE * sizeof(double2);
+    if (shmem > 220 * 1024) return fail(ctx, OV_EINVAL, "rotate_inplace: basis too large (%d vectors)", m);
+    if (ncol > m) return fail(ctx, OV_EINVAL, "rotate_inplace: ncol > m");
+    OV_CUDA(ctx, cudaFuncSetAttribute(rotate_inplace_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shmem));
+    const unsigned blocks = (unsigned)((n + kRotE - 1) / kRotE);
+    rotate_inplace_kernel<<<blocks, kRotThreads, shmem, ctx->stream>>>(a, na, b, stride, m, ncol, St_dev, n);
     ctx->launches++;
     OV_CUDA(ctx, cudaGetLastError());
     return OV_OK;

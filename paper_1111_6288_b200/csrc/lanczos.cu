@@ -6,6 +6,11 @@
 // Every filter term is two launches of the Wilson kernel with the three-term axpy in its epilogue, the same
 // fused step the Clenshaw recurrence uses.  A final Rayleigh-Ritz in Q itself separates +lambda from -lambda
 // and the true residuals |Q v - lambda v| are measured with the kernel (contract: <= tol, G13).
+//
+// Memory: the basis W[0..m] is the only large object.  Its first k vectors ARE the caller's output buffer, the rest is a
+// pool sized to what is free; restarts and the Rayleigh-Ritz step rotate the basis IN PLACE (rotate_inplace_kernel), so
+// k = 200 on 32^3x64 (80.5 GB of eigenvectors) runs in 180 GB with a Krylov space of ~1.5 k instead of needing a second
+// copy of the basis (the paper's 2.5 l subspace, would be 201 GB there).
 #include <algorithm>
 #include <cmath>
 #include <numeric>
@@ -54,41 +59,52 @@ static int apply_filter(ov_ctx* ctx, const Filter& f, const double2* in, double2
     return OV_OK;
 }
 
+// The Lanczos basis in two segments: vectors 0..na-1 in the caller's output buffer, the rest in the pool.
+struct Basis {
+    double2* a; int na; double2* b; size_t n;
+    double2* vec(int i) const { return i < na ? a + (size_t)i * n : b + (size_t)(i - na) * n; }
+};
+
+// d_result[0..nv) = W[0..nv)^+ u
+static int basis_dots(ov_ctx* ctx, const Basis& W, int nv, const double2* u) {
+    const int n1 = std::min(nv, W.na), n2 = nv - n1;
+    OV_TRY(launch_multi_dot_at(ctx, W.a, W.n, n1, u, 0, nv));
+    if (n2 > 0) OV_TRY(launch_multi_dot_at(ctx, W.b, W.n, n2, u, n1, nv));
+    return OV_OK;
+}
+
+// u += sum_{first <= i < first+nv} C[i-first] W[i]   (C: nv complex on the device)
+static int basis_axpy(ov_ctx* ctx, const Basis& W, int first, int nv, const double2* d_C, double2* u) {
+    MultiAxpyOuts o;
+    o.out[0] = u; o.bscale[0] = 1.0;
+    const int n1 = std::max(0, std::min(first + nv, W.na) - first), n2 = nv - n1;
+    if (n1 > 0) OV_TRY(launch_multi_axpy(ctx, W.vec(first), W.n, n1, 1, d_C, u, o));
+    if (n2 > 0) OV_TRY(launch_multi_axpy(ctx, W.vec(first + n1), W.n, n2, 1, d_C + n1, u, o));
+    return OV_OK;
+}
+
 // u -= W[0..nv) (W^+ u), returns the coefficients (host) ; one classical Gram-Schmidt pass
-static int cgs_pass(ov_ctx* ctx, const double2* W, size_t stride, int nv, double2* u, double2* d_C,
-                    std::vector<double2>& c) {
-    OV_TRY(launch_multi_dot(ctx, W, stride, nv, u));
+static int cgs_pass(ov_ctx* ctx, const Basis& W, int nv, double2* u, double2* d_C, std::vector<double2>& c) {
+    OV_TRY(basis_dots(ctx, W, nv, u));
     c.resize(nv);
     OV_TRY(fetch_results(ctx, nv, c.data()));
     std::vector<double2> neg(nv);
     for (int i = 0; i < nv; i++) neg[i] = make_double2(-c[i].x, -c[i].y);
     OV_CUDA(ctx, cudaMemcpyAsync(d_C, neg.data(), nv * sizeof(double2), cudaMemcpyHostToDevice, ctx->stream));
     OV_CUDA(ctx, cudaStreamSynchronize(ctx->stream));  // neg is a stack-owned host buffer
-    MultiAxpyOuts o;
-    o.out[0] = u; o.bscale[0] = 1.0;
-    return launch_multi_axpy(ctx, W, stride, nv, 1, d_C, u, o);
+    return basis_axpy(ctx, W, 0, nv, d_C, u);
 }
 
-// Y[0..ncol) = W[0..m) S[:, cols]  (S row-major m x ldS, host) in blocks of up to 8 columns
-static int rotate(ov_ctx* ctx, const double2* W, size_t stride, int m, const std::vector<double2>& S, int ldS,
-                  const std::vector<int>& cols, double2* Y, double2* d_C) {
+// W[j] <- sum_{i<m} S[i][cols[j]] W[i], j < cols.size(), in place  (S row-major m x ldS, host)
+static int rotate(ov_ctx* ctx, const Basis& W, int m, const std::vector<double2>& S, int ldS, const std::vector<int>& cols,
+                  double2* d_St) {
     const int ncol = (int)cols.size();
-    int done = 0;
-    std::vector<double2> C;
-    while (done < ncol) {
-        const int rem = ncol - done;
-        const int J = rem >= 8 ? 8 : rem >= 4 ? 4 : rem >= 2 ? 2 : 1;
-        C.assign((size_t)m * J, make_double2(0, 0));
-        for (int i = 0; i < m; i++)
-            for (int j = 0; j < J; j++) C[(size_t)i * J + j] = S[(size_t)i * ldS + cols[done + j]];
-        OV_CUDA(ctx, cudaMemcpyAsync(d_C, C.data(), C.size() * sizeof(double2), cudaMemcpyHostToDevice, ctx->stream));
-        OV_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-        MultiAxpyOuts o;
-        for (int j = 0; j < J; j++) o.out[j] = Y + (size_t)(done + j) * stride;
-        OV_TRY(launch_multi_axpy(ctx, W, stride, m, J, d_C, nullptr, o));
-        done += J;
-    }
-    return OV_OK;
+    std::vector<double2> St((size_t)ncol * m);
+    for (int j = 0; j < ncol; j++)
+        for (int i = 0; i < m; i++) St[(size_t)j * m + i] = S[(size_t)i * ldS + cols[j]];
+    OV_CUDA(ctx, cudaMemcpyAsync(d_St, St.data(), St.size() * sizeof(double2), cudaMemcpyHostToDevice, ctx->stream));
+    OV_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return launch_rotate_inplace(ctx, W.a, W.na, W.b, W.n, m, ncol, d_St);
 }
 
 static double inverse_filter(const Filter& f, double theta_abs) {
@@ -111,21 +127,34 @@ extern "C" int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_resta
     const size_t n = spinor_elems(ctx), bytes = n * sizeof(double2);
     const long long dim = (long long)n;
     const int keep = k + std::max(8, k / 4);                    // wanted + buffer kept at every restart
+    const int m_min = keep + 8;
     int m = subspace > 0 ? subspace : 2 * k + 16;
-    if (m < keep + 8) m = keep + 8;
+    if (m < m_min) m = m_min;
     if ((long long)m >= dim) return fail(ctx, OV_EINVAL, "subspace %d too large for dimension %lld", m, dim);
+    if ((size_t)m * kRotTileBytesPerVector > 220 * 1024) m = (int)(220 * 1024 / kRotTileBytesPerVector);
+    {   // fit the pool into free memory: vectors k..m of the basis + 3 scratch (+ 2 GB head room for the workspaces)
+        size_t free_b = 0, total_b = 0;
+        OV_CUDA(ctx, cudaMemGetInfo(&free_b, &total_b));
+        const size_t head = (size_t)2 << 30;
+        const long long fit = free_b > head ? (long long)((free_b - head) / bytes) - 4 : 0;   // pool vectors available
+        if (subspace <= 0 && (long long)(m + 1 - k) > fit) m = (int)(fit + k - 1);
+        if (m < m_min) return fail(ctx, OV_ENOMEM, "lanczos: %d basis vectors do not fit in free device memory", m_min + 1);
+    }
 
-    double2* pool = nullptr;  // W[0..m], Y[0..keep), 3 scratch
-    const size_t nvec = (size_t)m + 1 + keep + 3;
-    OV_CUDA(ctx, cudaMalloc(&pool, bytes * nvec));
-    double2* d_C = nullptr;
-    if (cudaMalloc(&d_C, (size_t)m * 8 * sizeof(double2)) != cudaSuccess) { cudaFree(pool); return fail(ctx, OV_ENOMEM, "lanczos: out of memory"); }
-    struct Free { double2 *a, *b; ~Free() { cudaFree(a); cudaFree(b); } } guard{pool, d_C};
-    double2* W = pool;
-    double2* Y = pool + (size_t)(m + 1) * n;
-    double2* t0 = Y + (size_t)keep * n;
-    double2* t1 = t0 + n;
+    double2* pool = nullptr;  // basis vectors k..m, then 3 scratch
+    const size_t npool = (size_t)(m + 1 - k) + 3;
+    OV_CUDA(ctx, cudaMalloc(&pool, bytes * npool));
+    double2 *d_C = nullptr, *d_St = nullptr;
+    if (cudaMalloc(&d_C, (size_t)(m + 1) * sizeof(double2)) != cudaSuccess ||
+        cudaMalloc(&d_St, (size_t)m * keep * sizeof(double2)) != cudaSuccess) {
+        cudaFree(pool); cudaFree(d_C);
+        return fail(ctx, OV_ENOMEM, "lanczos: out of memory");
+    }
+    struct Free { double2 *a, *b, *c; ~Free() { cudaFree(a); cudaFree(b); cudaFree(c); } } guard{pool, d_C, d_St};
+    const Basis W{(double2*)V_out_dev, k, pool, n};
+    double2* t1 = pool + (size_t)(m + 1 - k) * n;
     double2* tq = t1 + n;
+    double2* t0 = tq + n;
 
     auto normalise = [&](double2* v, double* nrm) -> int {
         double s;
@@ -135,10 +164,10 @@ extern "C" int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_resta
     };
 
     // ---- phase 0: a few plain Lanczos steps on A = Q^2 for an upper bound on lambda_min^2
-    random_fill_kernel<<<(unsigned)((dim + 255) / 256), 256, 0, ctx->stream>>>(W, dim, 0x1111628800ull);
+    random_fill_kernel<<<(unsigned)((dim + 255) / 256), 256, 0, ctx->stream>>>(W.vec(0), dim, 0x1111628800ull);
     ctx->launches++;
     double nrm;
-    OV_TRY(normalise(W, &nrm));
+    OV_TRY(normalise(W.vec(0), &nrm));
     double theta_min;
     {
         const int m0 = std::min(m, 40);
@@ -147,13 +176,13 @@ extern "C" int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_resta
         std::vector<double2> c;
         const double inv = 1.0 / ctx->norm;
         for (int j = 0; j < m0; j++) {
-            double2* u = W + (size_t)(j + 1) * n;
+            double2* u = W.vec(j + 1);
             Epilogue e1; e1.s = inv;
-            OV_TRY(launch_wilson(ctx, W + (size_t)j * n, tq, e1));
+            OV_TRY(launch_wilson(ctx, W.vec(j), tq, e1));
             OV_TRY(launch_wilson(ctx, tq, u, e1));
-            OV_TRY(cgs_pass(ctx, W, n, j + 1, u, d_C, c));
+            OV_TRY(cgs_pass(ctx, W, j + 1, u, d_C, c));
             double alpha = c[j].x;
-            OV_TRY(cgs_pass(ctx, W, n, j + 1, u, d_C, c));
+            OV_TRY(cgs_pass(ctx, W, j + 1, u, d_C, c));
             alpha += c[j].x;
             T[(size_t)j * m0 + j].x = alpha;
             OV_TRY(normalise(u, &nrm));
@@ -164,21 +193,20 @@ extern "C" int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_resta
     }
     Filter f{cheb_order, std::min(4.0 * theta_min, 0.5), 1.0};
 
-    std::vector<double2> T((size_t)m * m), S, c;
+    std::vector<double2> T((size_t)m * m, make_double2(0, 0)), S, c;
     std::vector<double> th;
     int l = 0;            // kept Ritz vectors at the front of W
     double tolB = 0.1 * tol;
     bool refined_filter = false;
     int rc_final = OV_ENOCONV;
-    std::fill(T.begin(), T.end(), make_double2(0, 0));
     // start vector: W[0] stays (normalised random)
     for (int restart = 0; restart < max_restarts; restart++) {
         for (int j = l; j < m; j++) {
-            double2* u = W + (size_t)(j + 1) * n;
-            OV_TRY(apply_filter(ctx, f, W + (size_t)j * n, u, t0, t1, tq));
-            OV_TRY(cgs_pass(ctx, W, n, j + 1, u, d_C, c));
+            double2* u = W.vec(j + 1);
+            OV_TRY(apply_filter(ctx, f, W.vec(j), u, t0, t1, tq));
+            OV_TRY(cgs_pass(ctx, W, j + 1, u, d_C, c));
             double alpha = c[j].x;
-            OV_TRY(cgs_pass(ctx, W, n, j + 1, u, d_C, c));
+            OV_TRY(cgs_pass(ctx, W, j + 1, u, d_C, c));
             alpha += c[j].x;
             T[(size_t)j * m + j] = make_double2(alpha, 0);
             OV_TRY(normalise(u, &nrm));
@@ -197,8 +225,15 @@ extern "C" int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_resta
             const double res = beta_last * std::hypot(s.x, s.y);
             if (res > tolB * std::fabs(th[kept[i]])) { conv = false; break; }
         }
-        // Ritz vectors of the kept set
-        OV_TRY(rotate(ctx, W, n, m, S, m, kept, Y, d_C));
+        // Ritz vectors of the kept set, in place: W[0..keep) <- W[0..m) S[:, kept]
+        OV_TRY(rotate(ctx, W, m, S, m, kept, d_St));
+        // projected matrix in the rotated basis: diag(theta) + the coupling to the residual vector W[m]
+        std::vector<double2> Tk((size_t)keep * keep, make_double2(0, 0)), zk(keep);
+        for (int i = 0; i < keep; i++) {
+            Tk[(size_t)i * keep + i] = make_double2(th[kept[i]], 0);
+            const double2 s = S[(size_t)(m - 1) * m + kept[i]];
+            zk[i] = make_double2(beta_last * s.x, -beta_last * s.y);   // T[i][keep]
+        }
 
         if (!refined_filter) {
             // tighten the filter edge to just above the kept set, restart the Krylov space from the Ritz vectors
@@ -209,9 +244,8 @@ extern "C" int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_resta
                 std::vector<double2> ones((size_t)keep, make_double2(1.0, 0.0));
                 OV_CUDA(ctx, cudaMemcpyAsync(d_C, ones.data(), keep * sizeof(double2), cudaMemcpyHostToDevice, ctx->stream));
                 OV_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-                MultiAxpyOuts o; o.out[0] = W;
-                OV_TRY(launch_multi_axpy(ctx, Y, n, keep, 1, d_C, nullptr, o));
-                OV_TRY(normalise(W, &nrm));
+                OV_TRY(basis_axpy(ctx, W, 1, keep - 1, d_C, W.vec(0)));   // W[0] = sum of the kept Ritz vectors
+                OV_TRY(normalise(W.vec(0), &nrm));
                 std::fill(T.begin(), T.end(), make_double2(0, 0));
                 l = 0;
                 continue;
@@ -219,13 +253,13 @@ extern "C" int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_resta
         }
 
         if (conv) {
-            // Rayleigh-Ritz in Q on span(Y): M = Y^+ Q Y
+            // Rayleigh-Ritz in Q on span(W[0..keep)): M = Y^+ Q Y
             std::vector<double2> M((size_t)keep * keep), SM;
             std::vector<double> mu;
             Epilogue eq; eq.s = 1.0 / ctx->norm;
             for (int j = 0; j < keep; j++) {
-                OV_TRY(launch_wilson(ctx, Y + (size_t)j * n, tq, eq));
-                OV_TRY(launch_multi_dot(ctx, Y, n, keep, tq));
+                OV_TRY(launch_wilson(ctx, W.vec(j), tq, eq));
+                OV_TRY(basis_dots(ctx, W, keep, tq));
                 c.resize(keep);
                 OV_TRY(fetch_results(ctx, keep, c.data()));
                 for (int i = 0; i < keep; i++) M[(size_t)i * keep + j] = c[i];
@@ -238,38 +272,59 @@ extern "C" int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_resta
                     M[(size_t)j * keep + i] = make_double2(h.x, -h.y);
                 }
             host_eigh(keep, M, mu, SM);
-            std::vector<int> sel(keep);
-            std::iota(sel.begin(), sel.end(), 0);
-            std::sort(sel.begin(), sel.end(), [&](int a, int b2) { return std::fabs(mu[a]) < std::fabs(mu[b2]); });
-            sel.resize(k);
-            double2* Vout = (double2*)V_out_dev;
-            OV_TRY(rotate(ctx, Y, n, keep, SM, keep, sel, Vout, d_C));
+            std::vector<int> order(keep);
+            std::iota(order.begin(), order.end(), 0);
+            std::sort(order.begin(), order.end(), [&](int a, int b2) { return std::fabs(mu[a]) < std::fabs(mu[b2]); });
+            // rotate the whole kept block by the unitary R = SM[:, order], in place: the wanted k eigenvectors of Q land in
+            // W[0..k) = the caller's buffer, and W[0..keep) stays an orthonormal basis of the same space
+            OV_TRY(rotate(ctx, W, keep, SM, keep, order, d_St));
             double worst = 0.0;
             for (int i = 0; i < k; i++) {
-                double2* v = Vout + (size_t)i * n;
+                double2* v = W.vec(i);
                 double nv;
                 OV_TRY(normalise(v, &nv));
-                Epilogue er; er.s = 1.0 / ctx->norm; er.A1 = v; er.a1 = -mu[sel[i]];
+                Epilogue er; er.s = 1.0 / ctx->norm; er.A1 = v; er.a1 = -mu[order[i]];
                 OV_TRY(launch_wilson(ctx, v, tq, er));
                 double r2;
                 OV_TRY(norm2_host(ctx, tq, &r2));
-                lambda_out_host[i] = mu[sel[i]];
+                lambda_out_host[i] = mu[order[i]];
                 resid_out_host[i] = std::sqrt(r2);
                 worst = std::max(worst, resid_out_host[i]);
             }
             if (worst <= tol) { rc_final = OV_OK; break; }
-            tolB *= 0.1;  // not there yet: ask more of the Krylov space and go on
+            tolB *= 0.1;  // not there yet: ask more of the Krylov space and go on, in the rotated basis
+            std::vector<double2> R((size_t)keep * keep), tmp((size_t)keep * keep), z2(keep);
+            for (int i = 0; i < keep; i++)
+                for (int j = 0; j < keep; j++) R[(size_t)i * keep + j] = SM[(size_t)i * keep + order[j]];
+            auto mul = [](double2 a, double2 b2) { return make_double2(a.x * b2.x - a.y * b2.y, a.x * b2.y + a.y * b2.x); };
+            auto cj = [](double2 a) { return make_double2(a.x, -a.y); };
+            for (int i = 0; i < keep; i++)       // tmp = Tk R   (Tk is diagonal here)
+                for (int j = 0; j < keep; j++) tmp[(size_t)i * keep + j] = mul(Tk[(size_t)i * keep + i], R[(size_t)i * keep + j]);
+            for (int a = 0; a < keep; a++) {     // Tk' = R^+ tmp ; z' = R^+ z
+                double2 za = make_double2(0, 0);
+                for (int i = 0; i < keep; i++) { const double2 p = mul(cj(R[(size_t)i * keep + a]), zk[i]); za.x += p.x; za.y += p.y; }
+                z2[a] = za;
+            }
+            std::vector<double2> Tn((size_t)keep * keep, make_double2(0, 0));
+            for (int a = 0; a < keep; a++)
+                for (int i = 0; i < keep; i++) {
+                    const double2 ra = cj(R[(size_t)i * keep + a]);
+                    for (int b2 = 0; b2 < keep; b2++) {
+                        const double2 p = mul(ra, tmp[(size_t)i * keep + b2]);
+                        Tn[(size_t)a * keep + b2].x += p.x; Tn[(size_t)a * keep + b2].y += p.y;
+                    }
+                }
+            Tk.swap(Tn);
+            zk.swap(z2);
         }
 
-        // thick restart: W[0..keep) = Y, W[keep] = W[m], T = diag(theta) + arrow
-        OV_CUDA(ctx, cudaMemcpyAsync(W, Y, bytes * (size_t)keep, cudaMemcpyDeviceToDevice, ctx->stream));
-        OV_CUDA(ctx, cudaMemcpyAsync(W + (size_t)keep * n, W + (size_t)m * n, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
+        // thick restart: W[0..keep) holds the kept vectors, W[keep] = W[m], T = [Tk z; z^+ .]
+        OV_CUDA(ctx, cudaMemcpyAsync(W.vec(keep), W.vec(m), bytes, cudaMemcpyDeviceToDevice, ctx->stream));
         std::fill(T.begin(), T.end(), make_double2(0, 0));
         for (int i = 0; i < keep; i++) {
-            T[(size_t)i * m + i] = make_double2(th[kept[i]], 0);
-            const double2 s = S[(size_t)(m - 1) * m + kept[i]];
-            T[(size_t)i * m + keep] = make_double2(beta_last * s.x, -beta_last * s.y);
-            T[(size_t)keep * m + i] = make_double2(beta_last * s.x, beta_last * s.y);
+            for (int j = 0; j < keep; j++) T[(size_t)i * m + j] = Tk[(size_t)i * keep + j];
+            T[(size_t)i * m + keep] = zk[i];
+            T[(size_t)keep * m + i] = make_double2(zk[i].x, -zk[i].y);
         }
         l = keep;
     }

@@ -12,6 +12,7 @@
 namespace ov {
 
 constexpr int kSpinorComplex = 12;  // 4 spins x 3 colours
+constexpr size_t kRotTileBytesPerVector = 16 * sizeof(double2);  // rotate_inplace_kernel: kRotE elements per vector
 
 // Internal gauge layout.  Default: planes [mu][e][V] double2.  -DOV_GAUGE_BLOCKED selects [V/32][mu][e][32 sites] (the
 // 4 links of a warp's 32 consecutive sites contiguous in HBM); it measured +3% on a cold burst of the Wilson kernel at
@@ -137,6 +138,12 @@ int launch_zero(ov_ctx* ctx, double2* x);
 int launch_gamma5(ov_ctx* ctx, const double2* x, double2* y);  // y = gamma5 x (may alias)
 // nvec dots <x_j, y> for j < nvec, x_j = xs + j*stride (complex results on device in ctx->d_result[0..nvec))
 int launch_multi_dot(ov_ctx* ctx, const double2* xs, size_t stride, int nvec, const double2* y);
+// same, results written to d_result[result_offset .. result_offset + nvec)
+int launch_multi_dot_at(ov_ctx* ctx, const double2* xs, size_t stride, int nvec, const double2* y, int result_offset,
+                        int result_total);
+// W[j] <- sum_i S[i][j] W[i], j < ncol, in place; basis in two segments (a: na vectors, b: the rest); St = S^T on device
+int launch_rotate_inplace(ov_ctx* ctx, double2* a, int na, double2* b, size_t stride, int m, int ncol,
+                          const double2* St_dev);
 int fetch_results(ov_ctx* ctx, int n, double2* host_out);  // sync + copy d_result[0..n) to host
 int dot_host(ov_ctx* ctx, const double2* x, const double2* y, double2* out);
 int norm2_host(ov_ctx* ctx, const double2* x, double* out);
