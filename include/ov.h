@@ -23,9 +23,13 @@
  * Layouts
  *   canonical gauge   complex128 [T][Z][Y][X][mu][row][col]   U_mu(x) links x -> x+mu
  *   canonical spinor  complex128 [T][Z][Y][X][spin][colour]   (= [site][12])
- *   ABI spinor ("SoA") complex128 [12][V]: component (spin s, colour c) of site i at complex index
- *                     (3*s+c)*V + i, (re,im) interleaved.  nrhs vectors are consecutive (stride 12*V).
- *                     ov_pack_spinor / ov_unpack_spinor convert canonical <-> ABI on the device.
+ *   ABI spinor        12*V complex128, site-major SoA in one of two forms, fixed per context (ov_spinor_layout):
+ *                       1 "blocked" (whenever V is a multiple of 32): component q = 3*spin+colour of site i at complex
+ *                         index ((i/32)*12 + q)*32 + i%32   -- 32-site blocks, components of a block contiguous;
+ *                       0 "planes" (any other V): component q of site i at q*V + i.
+ *                     (re,im) interleaved; nrhs vectors are consecutive (stride 12*V).  Callers normally never index
+ *                     it: ov_pack_spinor / ov_unpack_spinor convert canonical <-> ABI on the device, and every
+ *                     BLAS-1 / projector entry point is layout-agnostic.
  */
 #ifndef OV_H_
 #define OV_H_
@@ -60,6 +64,7 @@ void ov_destroy(ov_ctx* ctx);
 const char* ov_last_error(const ov_ctx* ctx);
 size_t ov_spinor_bytes(const ov_ctx* ctx); /* 192 * V */
 long long ov_volume(const ov_ctx* ctx);
+int ov_spinor_layout(const ov_ctx* ctx); /* 1 = blocked, 0 = planes (see Layouts above) */
 /* number of CUDA kernels this context has launched since creation (for bench.py's gpu_launches) */
 long long ov_launch_count(const ov_ctx* ctx);
 /* live timing for bench.py's roofline (CUDA events on the context's stream, recorded inside the calls that

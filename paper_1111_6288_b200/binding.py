@@ -20,7 +20,7 @@ _CODES = {1: "OV_EINVAL", 2: "OV_ENOMEM", 3: "OV_ECUDA", 4: "OV_ESTATE", 5: "OV_
 
 # every symbol include/ov.h declares (tests check that the library exports all of them)
 SYMBOLS = [
-    "ov_create", "ov_destroy", "ov_last_error", "ov_spinor_bytes", "ov_volume", "ov_launch_count",
+    "ov_create", "ov_destroy", "ov_last_error", "ov_spinor_bytes", "ov_volume", "ov_spinor_layout", "ov_launch_count",
     "ov_timing_enable", "ov_timing_read",
     "ov_set_dslash_variant", "ov_pack_spinor", "ov_unpack_spinor", "ov_dslash", "ov_apply_hw",
     "ov_chebyshev_coeffs", "ov_set_polynomial", "ov_set_smallspace", "ov_project", "ov_apply_sign",
@@ -137,6 +137,11 @@ class Overlap:
     @staticmethod
     def _nrhs(t):
         return 1 if t.dim() == 2 else t.shape[0]
+
+    @property
+    def spinor_layout(self):
+        """1 = blocked [V/32][12][32], 0 = planes [12][V] (include/ov.h, Layouts)."""
+        return int(self.lib.ov_spinor_layout(self._ctx))
 
     @property
     def launch_count(self):

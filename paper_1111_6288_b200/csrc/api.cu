@@ -112,6 +112,9 @@ int ov_create(ov_ctx** out, const int dims[4], double kappa, const void* gauge_d
     ctx->lat.V = (long long)dims[0] * dims[1] * dims[2] * dims[3];
     ctx->kappa = kappa;
     ctx->recon = recon;
+#ifndef OV_FORCE_PLANES
+    ctx->blocked = (ctx->lat.V % 32) == 0;
+#endif
     ctx->stream = (cudaStream_t)cuda_stream;
     const size_t gbytes = gauge_elems(ctx->lat.V, recon) * sizeof(double2);
     cudaError_t e = cudaMalloc(&ctx->gauge, gbytes);
@@ -144,6 +147,7 @@ void ov_destroy(ov_ctx* ctx) {
 const char* ov_last_error(const ov_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
 size_t ov_spinor_bytes(const ov_ctx* ctx) { return ctx ? spinor_elems(ctx) * sizeof(double2) : 0; }
 long long ov_volume(const ov_ctx* ctx) { return ctx ? ctx->lat.V : 0; }
+int ov_spinor_layout(const ov_ctx* ctx) { return ctx && ctx->blocked ? 1 : 0; }
 long long ov_launch_count(const ov_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
 int ov_timing_enable(ov_ctx* ctx, int on) {

@@ -10,24 +10,27 @@ namespace ov {
 
 // ------------------------------------------------------------------------------------------ layout
 // canonical gauge [site][mu][9] -> internal layout (gauge_index, ov_internal.h)
-template <int NE>
+template <int NE, bool BL>
 __global__ void gauge_relayout_kernel(const double2* __restrict__ can, double2* __restrict__ g, long long V) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= V) return;
 #pragma unroll
     for (int mu = 0; mu < 4; mu++)
 #pragma unroll
-        for (int e = 0; e < NE; e++) g[gauge_index<NE>(V, mu, e, i)] = can[(i * 4 + mu) * 9 + e];
+        for (int e = 0; e < NE; e++) g[gauge_index<NE, BL>(V, mu, e, i)] = can[(i * 4 + mu) * 9 + e];
 }
 
 int launch_gauge_relayout(ov_ctx* ctx, const double2* canonical) {
     const long long V = ctx->lat.V;
     const int threads = 128;
     const unsigned blocks = (unsigned)((V + threads - 1) / threads);
-    if (ctx->recon == 12)
-        gauge_relayout_kernel<6><<<blocks, threads, 0, ctx->stream>>>(canonical, ctx->gauge, V);
-    else
-        gauge_relayout_kernel<9><<<blocks, threads, 0, ctx->stream>>>(canonical, ctx->gauge, V);
+    if (ctx->recon == 12) {
+        if (ctx->blocked) gauge_relayout_kernel<6, true><<<blocks, threads, 0, ctx->stream>>>(canonical, ctx->gauge, V);
+        else gauge_relayout_kernel<6, false><<<blocks, threads, 0, ctx->stream>>>(canonical, ctx->gauge, V);
+    } else {
+        if (ctx->blocked) gauge_relayout_kernel<9, true><<<blocks, threads, 0, ctx->stream>>>(canonical, ctx->gauge, V);
+        else gauge_relayout_kernel<9, false><<<blocks, threads, 0, ctx->stream>>>(canonical, ctx->gauge, V);
+    }
     ctx->launches++;
     OV_CUDA(ctx, cudaGetLastError());
     return OV_OK;
@@ -35,7 +38,7 @@ int launch_gauge_relayout(ov_ctx* ctx, const double2* canonical) {
 
 // canonical spinor [site][12] <-> ABI [12][site], staged through shared memory so both sides coalesce
 constexpr int kPackSites = 128;
-template <bool PACK>
+template <bool PACK, bool BL>
 __global__ void __launch_bounds__(kPackSites) pack_kernel(const double2* __restrict__ src,
                                                           double2* __restrict__ dst, long long V) {
     __shared__ double2 tile[kPackSites * 12 + 12];
@@ -46,11 +49,11 @@ __global__ void __launch_bounds__(kPackSites) pack_kernel(const double2* __restr
         __syncthreads();
         if ((int)threadIdx.x < n)
 #pragma unroll
-            for (int c = 0; c < 12; c++) dst[(long long)c * V + base + threadIdx.x] = tile[threadIdx.x * 12 + c];
+            for (int c = 0; c < 12; c++) dst[spinor_base<BL>(base + threadIdx.x) + c * spinor_stride<BL>(V)] = tile[threadIdx.x * 12 + c];
     } else {
         if ((int)threadIdx.x < n)
 #pragma unroll
-            for (int c = 0; c < 12; c++) tile[threadIdx.x * 12 + c] = src[(long long)c * V + base + threadIdx.x];
+            for (int c = 0; c < 12; c++) tile[threadIdx.x * 12 + c] = src[spinor_base<BL>(base + threadIdx.x) + c * spinor_stride<BL>(V)];
         __syncthreads();
         for (int j = threadIdx.x; j < n * 12; j += kPackSites) dst[base * 12 + j] = tile[j];
     }
@@ -58,14 +61,18 @@ __global__ void __launch_bounds__(kPackSites) pack_kernel(const double2* __restr
 
 int launch_pack(ov_ctx* ctx, const double2* canonical, double2* abi) {
     const long long V = ctx->lat.V;
-    pack_kernel<true><<<(unsigned)((V + kPackSites - 1) / kPackSites), kPackSites, 0, ctx->stream>>>(canonical, abi, V);
+    const unsigned blocks = (unsigned)((V + kPackSites - 1) / kPackSites);
+    if (ctx->blocked) pack_kernel<true, true><<<blocks, kPackSites, 0, ctx->stream>>>(canonical, abi, V);
+    else pack_kernel<true, false><<<blocks, kPackSites, 0, ctx->stream>>>(canonical, abi, V);
     ctx->launches++;
     OV_CUDA(ctx, cudaGetLastError());
     return OV_OK;
 }
 int launch_unpack(ov_ctx* ctx, const double2* abi, double2* canonical) {
     const long long V = ctx->lat.V;
-    pack_kernel<false><<<(unsigned)((V + kPackSites - 1) / kPackSites), kPackSites, 0, ctx->stream>>>(abi, canonical, V);
+    const unsigned blocks = (unsigned)((V + kPackSites - 1) / kPackSites);
+    if (ctx->blocked) pack_kernel<false, true><<<blocks, kPackSites, 0, ctx->stream>>>(abi, canonical, V);
+    else pack_kernel<false, false><<<blocks, kPackSites, 0, ctx->stream>>>(abi, canonical, V);
     ctx->launches++;
     OV_CUDA(ctx, cudaGetLastError());
     return OV_OK;
@@ -108,8 +115,8 @@ __global__ void __launch_bounds__(kEwThreads) axpby_kernel(double a, const doubl
     }
 }
 
-// y = gamma5 x : components 6..11 (spins 2,3) change sign.  n = 12 V, element e has component e / V.
-__global__ void __launch_bounds__(kEwThreads) gamma5_kernel(const double2* x, double2* y, long long V) {
+// y = gamma5 x : components 6..11 (spins 2,3) change sign.  Element e has component e / V (planes) or (e/32) % 12 (blocked).
+__global__ void __launch_bounds__(kEwThreads) gamma5_kernel(const double2* x, double2* y, long long V, int blocked) {
     const long long n = 12 * V;
     const long long base = (long long)blockIdx.x * (kEwThreads * kEw) + threadIdx.x;
 #pragma unroll
@@ -117,7 +124,8 @@ __global__ void __launch_bounds__(kEwThreads) gamma5_kernel(const double2* x, do
         const long long e = base + (long long)m * kEwThreads;
         if (e < n) {
             double2 v = x[e];
-            if (e >= 6 * V) { v.x = -v.x; v.y = -v.y; }
+            const bool lower = blocked ? ((e >> 5) % 12) >= 6 : e >= 6 * V;
+            if (lower) { v.x = -v.x; v.y = -v.y; }
             y[e] = v;
         }
     }
@@ -147,7 +155,7 @@ int launch_zero(ov_ctx* ctx, double2* x) {
 }
 int launch_gamma5(ov_ctx* ctx, const double2* x, double2* y) {
     const long long n = (long long)spinor_elems(ctx);
-    gamma5_kernel<<<ew_blocks(n), kEwThreads, 0, ctx->stream>>>(x, y, ctx->lat.V);
+    gamma5_kernel<<<ew_blocks(n), kEwThreads, 0, ctx->stream>>>(x, y, ctx->lat.V, ctx->blocked ? 1 : 0);
     ctx->launches++;
     OV_CUDA(ctx, cudaGetLastError());
     return OV_OK;

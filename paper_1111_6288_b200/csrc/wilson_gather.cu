@@ -5,9 +5,9 @@
 //   out = s * G (in - kappa * hop(in)) + a1*A1 + a2*A2 + a3*A3        (Epilogue, ov_internal.h)
 //   hop(in)(x) = sum_mu [ s+ (1-gamma_mu) U_mu(x) in(x+mu) + s- (1+gamma_mu) U_mu(x-mu)^+ in(x-mu) ]
 //
-// Layouts: spinor component c of site i at double2 index c*V + i; link entry e (row-major) of U_mu(i) at
-// gauge_index<NE>(V, mu, e, i) (ov_internal.h), NE = 9 (recon 18) or 6 (recon 12).  A warp reads 32 consecutive
-// double2 (512 B) per component or link entry: fully coalesced LDG.128.
+// Layouts (ov_internal.h: spinor_base / gauge_index; blocked when V % 32 == 0, planes otherwise), NE = 9 link entries
+// (recon 18) or 6 (recon 12).  Either way a warp reads 32 consecutive double2 (512 B) per component or link entry:
+// fully coalesced LDG.128.
 // Successive launches walk the lattice in opposite block order (GatherArgs::reverse): the spinor one launch wrote last
 // is what the next launch reads first, while it is still in the 126 MB L2.
 #include "ov_internal.h"
@@ -31,31 +31,34 @@ struct GatherArgs {
 constexpr int kGatherThreads = 64;
 constexpr int kGatherMinBlocks = 6;
 
-template <int RECON>
+template <int RECON, bool BL>
 __device__ __forceinline__ void load_link(const double2* __restrict__ gauge, long long V, int mu,
                                           long long site, double2* __restrict__ u) {
     constexpr int NE = RECON / 2;
-    const double2* p = gauge + gauge_index<NE>(V, mu, 0, site);
-    const long long es = kGaugeBlocked ? 32 : V;  // stride between entries
+    const double2* p = gauge + gauge_index<NE, BL>(V, mu, 0, site);
+    const long long es = BL ? 32 : V;  // stride between entries
 #pragma unroll
     for (int e = 0; e < NE; e++) u[e] = __ldg(p + (long long)e * es);
     if (RECON == 12) su3_row2(u);
 }
 
-template <int MU, int SIGMA, int RECON>
+template <int MU, int SIGMA, int RECON, bool BL>
 __device__ __forceinline__ void hop(double2* __restrict__ acc, const GatherArgs& a, long long nsite,
                                     long long lsite, double ph) {
     double2 psi[12], h[6], g[6], u[9];
 #pragma unroll
-    for (int c = 0; c < 12; c++) psi[c] = __ldg(a.in + (long long)c * a.V + nsite);
+    const double2* pn = a.in + spinor_base<BL>(nsite);
+    const long long cs = spinor_stride<BL>(a.V);
+#pragma unroll
+    for (int c = 0; c < 12; c++) psi[c] = __ldg(pn + c * cs);
     project<MU, SIGMA>(psi, h);
-    load_link<RECON>(a.gauge, a.V, MU, lsite, u);
+    load_link<RECON, BL>(a.gauge, a.V, MU, lsite, u);
     su3_mul<(SIGMA > 0)>(u, h, g);
     reconstruct_add<MU, SIGMA>(acc, g, ph);
 }
 
 // NA: number of epilogue operands A1..A_NA (always filled in order); NA = -1: hop only
-template <int RECON, int NA>
+template <int RECON, int NA, bool BL>
 __global__ void __launch_bounds__(kGatherThreads, kGatherMinBlocks) wilson_gather_kernel(const GatherArgs a) {
     const unsigned blk = a.reverse ? gridDim.x - 1 - blockIdx.x : blockIdx.x;
     const long long i = (long long)blk * blockDim.x + threadIdx.x;
@@ -75,33 +78,34 @@ __global__ void __launch_bounds__(kGatherThreads, kGatherMinBlocks) wilson_gathe
     {
         const long long ip = (x + 1 == a.X) ? i - (a.X - 1) * sX : i + sX;
         const long long im = (x == 0) ? i + (a.X - 1) * sX : i - sX;
-        hop<0, -1, RECON>(acc, a, ip, i, 1.0);
-        hop<0, +1, RECON>(acc, a, im, im, 1.0);
+        hop<0, -1, RECON, BL>(acc, a, ip, i, 1.0);
+        hop<0, +1, RECON, BL>(acc, a, im, im, 1.0);
     }
     {
         const long long ip = (y + 1 == a.Y) ? i - (a.Y - 1) * sY : i + sY;
         const long long im = (y == 0) ? i + (a.Y - 1) * sY : i - sY;
-        hop<1, -1, RECON>(acc, a, ip, i, 1.0);
-        hop<1, +1, RECON>(acc, a, im, im, 1.0);
+        hop<1, -1, RECON, BL>(acc, a, ip, i, 1.0);
+        hop<1, +1, RECON, BL>(acc, a, im, im, 1.0);
     }
     {
         const long long ip = (z + 1 == a.Z) ? i - (a.Z - 1) * sZ : i + sZ;
         const long long im = (z == 0) ? i + (a.Z - 1) * sZ : i - sZ;
-        hop<2, -1, RECON>(acc, a, ip, i, 1.0);
-        hop<2, +1, RECON>(acc, a, im, im, 1.0);
+        hop<2, -1, RECON, BL>(acc, a, ip, i, 1.0);
+        hop<2, +1, RECON, BL>(acc, a, im, im, 1.0);
     }
     {
         const bool wp = (t + 1 == a.T), wm = (t == 0);
         const long long ip = wp ? i - (a.T - 1) * sT : i + sT;
         const long long im = wm ? i + (a.T - 1) * sT : i - sT;
-        hop<3, -1, RECON>(acc, a, ip, i, wp ? -1.0 : 1.0);  // antiperiodic in time
-        hop<3, +1, RECON>(acc, a, im, im, wm ? -1.0 : 1.0);
+        hop<3, -1, RECON, BL>(acc, a, ip, i, wp ? -1.0 : 1.0);  // antiperiodic in time
+        hop<3, +1, RECON, BL>(acc, a, im, im, wm ? -1.0 : 1.0);
     }
 
     const Epilogue& ep = a.ep;
+    const long long ib = spinor_base<BL>(i), cs = spinor_stride<BL>(a.V);
     if (NA < 0) {
 #pragma unroll
-        for (int c = 0; c < 12; c++) a.out[(long long)c * a.V + i] = acc[c];
+        for (int c = 0; c < 12; c++) a.out[ib + c * cs] = acc[c];
         return;
     }
     const double slo = ep.g5 ? -ep.s : ep.s;
@@ -114,7 +118,7 @@ __global__ void __launch_bounds__(kGatherThreads, kGatherMinBlocks) wilson_gathe
         double2 own[CH], w1[CH], w2[CH], w3[CH];
 #pragma unroll
         for (int k = 0; k < CH; k++) {
-            const long long e = (long long)(c0 + k) * a.V + i;
+            const long long e = ib + (c0 + k) * cs;
             own[k] = __ldg(a.in + e);
             if (NA >= 1) w1[k] = ep.A1[e];
             if (NA >= 2) w2[k] = ep.A2[e];
@@ -129,7 +133,7 @@ __global__ void __launch_bounds__(kGatherThreads, kGatherMinBlocks) wilson_gathe
             if (NA >= 1) { const double f = (lo && (ep.a_g5 & 1)) ? -ep.a1 : ep.a1; v.x = fma(f, w1[k].x, v.x); v.y = fma(f, w1[k].y, v.y); }
             if (NA >= 2) { const double f = (lo && (ep.a_g5 & 2)) ? -ep.a2 : ep.a2; v.x = fma(f, w2[k].x, v.x); v.y = fma(f, w2[k].y, v.y); }
             if (NA >= 3) { const double f = (lo && (ep.a_g5 & 4)) ? -ep.a3 : ep.a3; v.x = fma(f, w3[k].x, v.x); v.y = fma(f, w3[k].y, v.y); }
-            a.out[(long long)c * a.V + i] = v;
+            a.out[ib + c * cs] = v;
         }
     }
 }
@@ -153,7 +157,11 @@ int launch_wilson_gather(ov_ctx* ctx, const double2* in, double2* out, const Epi
     const unsigned blocks = (unsigned)((a.V + threads - 1) / threads);
     const int na = ep.hop_only ? -1 : (ep.A3 ? 3 : ep.A2 ? 2 : ep.A1 ? 1 : 0);
     if ((ep.A3 && !ep.A2) || (ep.A2 && !ep.A1)) return fail(ctx, OV_EINVAL, "epilogue operands must be filled in order");
-#define OV_GATHER(R, N) wilson_gather_kernel<R, N><<<blocks, threads, 0, ctx->stream>>>(a)
+#define OV_GATHER(R, N)                                                                   \
+    do {                                                                                  \
+        if (ctx->blocked) wilson_gather_kernel<R, N, true><<<blocks, threads, 0, ctx->stream>>>(a);  \
+        else wilson_gather_kernel<R, N, false><<<blocks, threads, 0, ctx->stream>>>(a);   \
+    } while (0)
 #define OV_GATHER_NA(R)                                 \
     switch (na) {                                       \
         case -1: OV_GATHER(R, -1); break;               \

@@ -60,15 +60,25 @@ def test_pack_unpack_roundtrip(ovp):
     x = np.stack([wl.gaussian_source(dims, s) for s in (1, 2, 3)])
     d = to_dev(op, x)
     assert d.shape == (3, 12, op.V)
-    # ABI layout: component (3*s+c) of site i at [comp][i]
-    ref = x.reshape(3, op.V, 12).transpose(0, 2, 1)
+    # ABI layout (include/ov.h): V = 384 is a multiple of 32 -> blocked [V/32][12][32]
+    assert op.spinor_layout == 1
+    ref = x.reshape(3, op.V // 32, 32, 12).transpose(0, 1, 3, 2).reshape(3, 12, op.V)
     assert np.array_equal(d.cpu().numpy(), ref)
     assert np.array_equal(to_host(op, d), x)
+    # a volume that is not a multiple of 32 uses planes [12][V]
+    dims2 = (6, 6, 2, 2)
+    op2 = make(ovp, dims2, wl.unit_links(dims2))
+    x2 = wl.gaussian_source(dims2, 4)
+    d2 = to_dev(op2, x2)
+    assert op2.spinor_layout == 0
+    assert np.array_equal(d2.cpu().numpy(), x2.reshape(op2.V, 12).T)
+    assert np.array_equal(to_host(op2, d2), x2)
 
 
 # ------------------------------------------------------------------------------------------ Wilson kernel
 @pytest.mark.parametrize("dims,spread", [((4, 4, 4, 4), 0.3), ((4, 2, 6, 8), 0.6), ((8, 8, 8, 16), 0.5),
-                                         ((24, 4, 4, 2), 0.8), ((6, 10, 2, 4), 0.4)])
+                                         ((24, 4, 4, 2), 0.8), ((6, 10, 2, 4), 0.4), ((6, 6, 2, 6), 0.5),
+                                         ((2, 2, 2, 2), 0.7)])
 @pytest.mark.parametrize("recon", [18, 12])
 def test_dslash_and_hw_vs_oracle(ovp, dims, spread, recon):
     U = wl.su3_links(dims, spread, wl.gauge_seed(1))
