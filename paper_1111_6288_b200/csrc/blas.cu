@@ -3,6 +3,8 @@
 // HBM bandwidth, the design rule is 16-byte coalesced accesses and enough loads in flight per thread.
 // Reductions are two-stage with a fixed shape (warp shuffle -> per-warp partial in global memory ->
 // one block per result summing the partials in a fixed tree), no atomics: bit-reproducible.
+#include <algorithm>
+
 #include "ov_internal.h"
 #include "wilson_math.cuh"
 
@@ -162,44 +164,91 @@ int launch_gamma5(ov_ctx* ctx, const double2* x, double2* y) {
 }
 
 // ------------------------------------------------------------------------------------------ reductions
-// multi-dot: r_j = sum_e conj(x_j[e]) y[e], j < nvec.  Each warp owns kDotE*32 consecutive elements of y,
-// keeps them in registers, and streams the same window of every x_j once: y is read from HBM exactly
-// once however many vectors there are (the small-space V^+ x of PAPER.md:39/:81 with k = 100-200).
-constexpr int kDotE = 8;
+// multi-dot: r_j = sum_e conj(x_j[e]) y[e], j < nvec  (the small-space V^+ x of PAPER.md:39/:81 with k = 100-200).
+// A warp owns a window of kDotE*32 consecutive elements of y, keeps them in registers and streams the same window of
+// every x_j once, so y is read from HBM exactly once.  The vectors are taken four at a time: the loads of the next four
+// are issued before the current four are reduced (16 independent 16-byte loads in flight per lane), and the four complex
+// partial sums are reduced together by a halving butterfly (18 shuffles per 4 vectors instead of 80).  Warps park their
+// sums in shared memory; one fixed-order pass per block writes partial[j][block]: deterministic, no atomics.
+constexpr int kDotE = 2;
 constexpr int kDotThreads = 256;
-constexpr int kDotWarpElems = kDotE * 32;
+constexpr int kDotWarps = kDotThreads / 32;
+constexpr int kDotBlockElems = kDotE * kDotThreads;
+constexpr int kDotMaxVec = 1024;  // vectors per launch (shared memory: nvec * 8 warps * 16 B)
+
+__device__ __forceinline__ void dot_load4(const double2* __restrict__ xs, size_t stride, int j, int nvec, long long base,
+                                          long long n, double2 (&xv)[4][kDotE]) {
+#pragma unroll
+    for (int u = 0; u < 4; u++)
+#pragma unroll
+        for (int m = 0; m < kDotE; m++) {
+            const long long e = base + m * 32;
+            xv[u][m] = (j + u < nvec && e < n) ? __ldcs(xs + (size_t)(j + u) * stride + e) : make_double2(0.0, 0.0);
+        }
+}
 
 __global__ void __launch_bounds__(kDotThreads) multi_dot_kernel(const double2* __restrict__ xs, size_t stride,
                                                                 int nvec, const double2* __restrict__ y,
-                                                                long long n, long long nwarps,
+                                                                long long n, long long nblocks,
                                                                 double2* __restrict__ partial) {
-    const int lane = threadIdx.x & 31;
-    const long long warp = (long long)blockIdx.x * (kDotThreads / 32) + (threadIdx.x >> 5);
-    if (warp >= nwarps) return;
-    const long long base = warp * kDotWarpElems + lane;
+    extern __shared__ double2 sacc[];  // [nvec][kDotWarps]
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const long long base = (long long)blockIdx.x * kDotBlockElems + warp * (kDotE * 32) + lane;
     double2 yv[kDotE];
 #pragma unroll
     for (int m = 0; m < kDotE; m++) {
         const long long e = base + m * 32;
         yv[m] = (e < n) ? y[e] : make_double2(0.0, 0.0);
     }
-    for (int j = 0; j < nvec; j++) {
-        const double2* x = xs + (size_t)j * stride;
-        double2 xv[kDotE];
+    double2 cur[4][kDotE], nxt[4][kDotE];
+    dot_load4(xs, stride, 0, nvec, base, n, cur);
+    for (int j = 0; j < nvec; j += 4) {
+        dot_load4(xs, stride, j + 4, nvec, base, n, nxt);   // next four in flight while these are reduced
+        double v[8];
 #pragma unroll
-        for (int m = 0; m < kDotE; m++) {
-            const long long e = base + m * 32;
-            xv[m] = (e < n) ? __ldcs(x + e) : make_double2(0.0, 0.0);
+        for (int u = 0; u < 4; u++) {
+            double2 acc = make_double2(0.0, 0.0);
+#pragma unroll
+            for (int m = 0; m < kDotE; m++) cmaddc(acc, cur[u][m], yv[m]);
+            v[2 * u] = acc.x; v[2 * u + 1] = acc.y;
         }
-        double2 acc = make_double2(0.0, 0.0);
+        // halving butterfly: 8 -> 4 -> 2 -> 1 values per lane, then two plain steps
 #pragma unroll
-        for (int m = 0; m < kDotE; m++) cmaddc(acc, xv[m], yv[m]);
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            acc.x += __shfl_xor_sync(0xffffffffu, acc.x, o);
-            acc.y += __shfl_xor_sync(0xffffffffu, acc.y, o);
+        for (int q = 0; q < 4; q++) {
+            const bool up = lane & 16;
+            const double send = up ? v[q] : v[q + 4], keep = up ? v[q + 4] : v[q];
+            v[q] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
         }
-        if (lane == 0) partial[(long long)j * nwarps + warp] = acc;
+#pragma unroll
+        for (int q = 0; q < 2; q++) {
+            const bool up = lane & 8;
+            const double send = up ? v[q] : v[q + 2], keep = up ? v[q + 2] : v[q];
+            v[q] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+        }
+        {
+            const bool up = lane & 4;
+            const double send = up ? v[0] : v[1], keep = up ? v[1] : v[0];
+            v[0] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+        }
+        v[0] += __shfl_xor_sync(0xffffffffu, v[0], 2);
+        v[0] += __shfl_xor_sync(0xffffffffu, v[0], 1);
+        // lane l (l % 4 == 0) holds value index 4*bit4 + 2*bit3 + bit2 = (vector j + idx/2, re/im idx%2)
+        if ((lane & 3) == 0) {
+            const int idx = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
+            const int jj = j + (idx >> 1);
+            if (jj < nvec) reinterpret_cast<double*>(sacc + (size_t)jj * kDotWarps + warp)[idx & 1] = v[0];
+        }
+#pragma unroll
+        for (int u = 0; u < 4; u++)
+#pragma unroll
+            for (int m = 0; m < kDotE; m++) cur[u][m] = nxt[u][m];
+    }
+    __syncthreads();
+    for (int jj = threadIdx.x; jj < nvec; jj += kDotThreads) {
+        double2 t = sacc[(size_t)jj * kDotWarps];
+#pragma unroll
+        for (int w = 1; w < kDotWarps; w++) t = cadd(t, sacc[(size_t)jj * kDotWarps + w]);
+        partial[(long long)jj * nblocks + blockIdx.x] = t;
     }
 }
 
@@ -223,13 +272,19 @@ __global__ void __launch_bounds__(kRedThreads) reduce_partials_kernel(const doub
 int launch_multi_dot_at(ov_ctx* ctx, const double2* xs, size_t stride, int nvec, const double2* y, int result_offset,
                         int result_total) {
     const long long n = (long long)spinor_elems(ctx);
-    const long long nwarps = (n + kDotWarpElems - 1) / kDotWarpElems;
-    OV_TRY(ensure_reduction_buffers(ctx, (size_t)nwarps * result_total, (size_t)result_total));
-    const unsigned blocks = (unsigned)((nwarps + kDotThreads / 32 - 1) / (kDotThreads / 32));
-    double2* partial = ctx->d_partial + (size_t)result_offset * nwarps;
-    multi_dot_kernel<<<blocks, kDotThreads, 0, ctx->stream>>>(xs, stride, nvec, y, n, nwarps, partial);
-    reduce_partials_kernel<<<nvec, kRedThreads, 0, ctx->stream>>>(partial, nwarps, ctx->d_result + result_offset);
-    ctx->launches += 2;
+    const long long nblocks = (n + kDotBlockElems - 1) / kDotBlockElems;
+    OV_TRY(ensure_reduction_buffers(ctx, (size_t)nblocks * result_total, (size_t)result_total));
+    for (int j0 = 0; j0 < nvec; j0 += kDotMaxVec) {
+        const int nv = std::min(kDotMaxVec, nvec - j0);
+        const size_t shmem = (size_t)nv * kDotWarps * sizeof(double2);
+        if (shmem > 48 * 1024)
+            OV_CUDA(ctx, cudaFuncSetAttribute(multi_dot_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shmem));
+        double2* partial = ctx->d_partial + (size_t)(result_offset + j0) * nblocks;
+        multi_dot_kernel<<<(unsigned)nblocks, kDotThreads, shmem, ctx->stream>>>(xs + (size_t)j0 * stride, stride, nv, y, n,
+                                                                                  nblocks, partial);
+        reduce_partials_kernel<<<nv, kRedThreads, 0, ctx->stream>>>(partial, nblocks, ctx->d_result + result_offset + j0);
+        ctx->launches += 2;
+    }
     OV_CUDA(ctx, cudaGetLastError());
     return OV_OK;
 }
