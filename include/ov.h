@@ -114,6 +114,10 @@ int ov_project(ov_ctx* ctx, const void* in, void* perp, void* low, double* coef_
  * and copy the canonical result back (synchronous) -- the end-to-end entry point bench.py times.     */
 int ov_apply_sign(ov_ctx* ctx, const void* in, void* out, int nrhs);
 int ov_apply_dov(ov_ctx* ctx, double mass, const void* in, void* out, int nrhs);
+/* reduced-accuracy D_ov (the building block of the adaptive CG; also a test hook): the polynomial is the
+ * caller's Chebyshev series truncated to `order` <= the order set, and with use_f32 != 0 the Clenshaw sweep runs in
+ * single precision (links and Clenshaw vectors in fp32; projector, in, out and the D_ov assembly stay fp64).  One RHS. */
+int ov_apply_dov_reduced(ov_ctx* ctx, double mass, const void* in, void* out, int order, int use_f32);
 int ov_apply_hw_host(ov_ctx* ctx, const void* in_host, void* out_host, int nrhs);
 int ov_apply_dov_host(ov_ctx* ctx, double mass, const void* in_host, void* out_host, int nrhs);
 
@@ -140,6 +144,16 @@ int ov_blas_norm2(ov_ctx* ctx, const void* x, double* out_host);
  *   Memory: V_out_dev itself holds the first k basis vectors during the call (its contents are scratch until the
  *   call returns); the library allocates the other m+1-k basis vectors + 3 spinors and frees them before returning.
  *   All basis rotations are done in place, so k = 200 on 32^3x64 (80.5 GB of V) fits in 180 GB.                    */
+/* ov_set_cg_adaptive ("adaptive CG": lower polynomial order as the CG converges, then single precision):
+ *   mode 0 (default): every operator application at full order in fp64;
+ *   mode 1: at iteration j the application of A only needs relative accuracy eta_j ~ tol |b| / |r_j| (inexact-Krylov
+ *           relaxation), so the series is truncated to the smallest order whose difference from the full polynomial,
+ *           measured on [min(eps, lambda_k^2), 1], is below eta_j;
+ *   mode 2: mode 1, and the Clenshaw sweep runs in fp32 once eta_j is above the fp32 rounding floor.
+ * The CG vectors and recurrences stay fp64; the true residuals reported at the end always use the full operator. */
+int ov_set_cg_adaptive(ov_ctx* ctx, int mode);
+/* the order used at each iteration of the last adaptive solve (negative = fp32 sweep); returns the iteration count */
+int ov_cg_orders(const ov_ctx* ctx, int* out_host, int cap);
 int ov_multishift_cg(ov_ctx* ctx, const double* masses_host, int nmass, const void* b, void* x, double tol,
                      int maxiter, int* iters_out, double* relres_out);
 int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_restarts, int cheb_order, int subspace,

@@ -24,7 +24,7 @@ SYMBOLS = [
     "ov_timing_enable", "ov_timing_read",
     "ov_set_dslash_variant", "ov_pack_spinor", "ov_unpack_spinor", "ov_dslash", "ov_apply_hw",
     "ov_chebyshev_coeffs", "ov_set_polynomial", "ov_set_smallspace", "ov_project", "ov_apply_sign",
-    "ov_apply_dov", "ov_apply_hw_host", "ov_apply_dov_host", "ov_blas_axpy", "ov_blas_scale", "ov_blas_dot",
+    "ov_apply_dov", "ov_apply_dov_reduced", "ov_set_cg_adaptive", "ov_cg_orders", "ov_apply_hw_host", "ov_apply_dov_host", "ov_blas_axpy", "ov_blas_scale", "ov_blas_dot",
     "ov_blas_norm2", "ov_multishift_cg", "ov_lanczos_lowmodes", "ov_host_eigh",
 ]
 
@@ -193,6 +193,20 @@ class Overlap:
 
     def apply_dov(self, mass, x, out=None):
         return self._apply(self.lib.ov_apply_dov, x, out, ctypes.c_double(mass))
+
+    def apply_dov_reduced(self, mass, x, order, use_f32, out=None):
+        out = torch.empty_like(x) if out is None else out
+        self._check(self.lib.ov_apply_dov_reduced(self._ctx, ctypes.c_double(mass), _ptr(x), _ptr(out), ctypes.c_int(order),
+                                                  ctypes.c_int(1 if use_f32 else 0)))
+        return out
+
+    def set_cg_adaptive(self, mode):
+        self._check(self.lib.ov_set_cg_adaptive(self._ctx, ctypes.c_int(mode)))
+
+    def cg_orders(self):
+        buf = (ctypes.c_int * 4096)()
+        n = self.lib.ov_cg_orders(self._ctx, buf, ctypes.c_int(4096))
+        return [buf[i] for i in range(min(n, 4096))]
 
     def apply_hw_host(self, x_host: np.ndarray) -> np.ndarray:
         """canonical HOST array in, canonical HOST array out (H2D and D2H inside the call)."""

@@ -27,6 +27,12 @@ int workspace(ov_ctx* ctx, int i, double2** out) {
     return OV_OK;
 }
 
+int workspace_f32(ov_ctx* ctx, int i, float2** out) {
+    if (!ctx->wsf[i]) OV_CUDA(ctx, cudaMalloc(&ctx->wsf[i], spinor_elems(ctx) * sizeof(float2)));
+    *out = ctx->wsf[i];
+    return OV_OK;
+}
+
 int ensure_reduction_buffers(ov_ctx* ctx, size_t partial_elems, size_t result_elems) {
     if (partial_elems > ctx->partial_cap) {
         OV_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
@@ -132,6 +138,8 @@ void ov_destroy(ov_ctx* ctx) {
     cudaStreamSynchronize(ctx->stream);
     cudaFree(ctx->gauge);
     for (auto& w : ctx->ws) cudaFree(w);
+    for (auto& w : ctx->wsf) cudaFree(w);
+    cudaFree(ctx->gauge_f);
     cudaFree(ctx->d_partial);
     cudaFree(ctx->d_result);
     if (ctx->h_result) cudaFreeHost(ctx->h_result);

@@ -111,6 +111,25 @@ int ov_apply_dov(ov_ctx* ctx, double mass, const void* in, void* out, int nrhs) 
     return OV_OK;
 }
 
+int ov_apply_dov_reduced(ov_ctx* ctx, double mass, const void* in, void* out, int order, int use_f32) {
+    OV_TRY(check2(ctx, in, out, 1));
+    return apply_dov_reduced(ctx, mass, (const double2*)in, (double2*)out, order, use_f32 != 0);
+}
+
+int ov_set_cg_adaptive(ov_ctx* ctx, int mode) {
+    if (!ctx) return OV_EINVAL;
+    if (mode < 0 || mode > 2) return fail(ctx, OV_EINVAL, "mode must be 0, 1 or 2");
+    ctx->cg_adaptive = mode;
+    return OV_OK;
+}
+
+int ov_cg_orders(const ov_ctx* ctx, int* out_host, int cap) {
+    if (!ctx) return 0;
+    const int n = (int)ctx->cg_orders.size();
+    for (int i = 0; i < n && i < cap && out_host; i++) out_host[i] = ctx->cg_orders[i];
+    return n;
+}
+
 // host-buffer path: H2D -> pack -> operator -> unpack -> D2H, one RHS at a time through 3 device stages
 static int host_apply(ov_ctx* ctx, int which, double mass, const void* in_host, void* out_host, int nrhs) {
     if (!ctx) return OV_EINVAL;

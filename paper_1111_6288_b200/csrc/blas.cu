@@ -432,3 +432,77 @@ int launch_rotate_inplace(ov_ctx* ctx, double2* a, int na, double2* b, size_t st
 }
 
 }  // namespace ov
+
+namespace ov {
+
+// ------------------------------------------------------------------------------------------ fp32 helpers
+// The reduced-precision tail of the adaptive CG keeps every CG vector in fp64 and runs only the Clenshaw
+// sweep of an operator application in fp32: y32 = (float) a*x on the way in, out = r32 + a1*A1 + a2*[gamma5]A2 on the
+// way out (both fp64 operands; the D_ov assembly of row a5).
+__global__ void __launch_bounds__(kEwThreads) scale_to_f32_kernel(double a, const double2* __restrict__ x,
+                                                                  float2* __restrict__ y, long long n) {
+    const long long base = (long long)blockIdx.x * (kEwThreads * kEw) + threadIdx.x;
+#pragma unroll
+    for (int m = 0; m < kEw; m++) {
+        const long long e = base + (long long)m * kEwThreads;
+        if (e < n) { const double2 v = x[e]; y[e] = make_float2((float)(a * v.x), (float)(a * v.y)); }
+    }
+}
+
+__global__ void __launch_bounds__(kEwThreads) combine_from_f32_kernel(const float2* __restrict__ r, double a1,
+                                                                      const double2* __restrict__ A1, double a2,
+                                                                      const double2* __restrict__ A2, int a2_g5,
+                                                                      double2* out, long long V, int blocked) {
+    const long long n = 12 * V;
+    const long long base = (long long)blockIdx.x * (kEwThreads * kEw) + threadIdx.x;
+#pragma unroll
+    for (int m = 0; m < kEw; m++) {
+        const long long e = base + (long long)m * kEwThreads;
+        if (e < n) {
+            const float2 rf = r[e];
+            double2 v = make_double2((double)rf.x, (double)rf.y);
+            if (A1) { const double2 w = A1[e]; v.x = fma(a1, w.x, v.x); v.y = fma(a1, w.y, v.y); }
+            if (A2) {
+                const bool lower = blocked ? ((e >> 5) % 12) >= 6 : e >= 6 * V;
+                const double f = (a2_g5 && lower) ? -a2 : a2;
+                const double2 w = A2[e]; v.x = fma(f, w.x, v.x); v.y = fma(f, w.y, v.y);
+            }
+            out[e] = v;
+        }
+    }
+}
+
+__global__ void __launch_bounds__(kEwThreads) gauge_to_f32_kernel(const double2* __restrict__ g, float2* __restrict__ gf,
+                                                                  long long n) {
+    const long long e = (long long)blockIdx.x * kEwThreads + threadIdx.x;
+    if (e < n) { const double2 v = g[e]; gf[e] = make_float2((float)v.x, (float)v.y); }
+}
+
+int launch_scale_to_f32(ov_ctx* ctx, double a, const double2* x, float2* y) {
+    const long long n = (long long)spinor_elems(ctx);
+    scale_to_f32_kernel<<<ew_blocks(n), kEwThreads, 0, ctx->stream>>>(a, x, y, n);
+    ctx->launches++;
+    OV_CUDA(ctx, cudaGetLastError());
+    return OV_OK;
+}
+int launch_combine_from_f32(ov_ctx* ctx, const float2* r, double a1, const double2* A1, double a2, const double2* A2,
+                            int a2_g5, double2* out) {
+    const long long n = (long long)spinor_elems(ctx);
+    combine_from_f32_kernel<<<ew_blocks(n), kEwThreads, 0, ctx->stream>>>(r, a1, A1, a2, A2, a2_g5, out, ctx->lat.V,
+                                                                          ctx->blocked ? 1 : 0);
+    ctx->launches++;
+    OV_CUDA(ctx, cudaGetLastError());
+    return OV_OK;
+}
+// fp32 copy of the links (same layout as the fp64 ones), made once on first use
+int ensure_gauge_f32(ov_ctx* ctx) {
+    if (ctx->gauge_f) return OV_OK;
+    const long long n = (long long)gauge_elems(ctx->lat.V, ctx->recon);
+    OV_CUDA(ctx, cudaMalloc(&ctx->gauge_f, (size_t)n * sizeof(float2)));
+    gauge_to_f32_kernel<<<(unsigned)((n + kEwThreads - 1) / kEwThreads), kEwThreads, 0, ctx->stream>>>(ctx->gauge, ctx->gauge_f, n);
+    ctx->launches++;
+    OV_CUDA(ctx, cudaGetLastError());
+    return OV_OK;
+}
+
+}  // namespace ov

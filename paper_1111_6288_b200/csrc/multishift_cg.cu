@@ -18,6 +18,37 @@ static int apply_A(ov_ctx* ctx, const double2* in, double2* tmp, double2* out) {
     return launch_gamma5(ctx, out, out);
 }
 
+// same at reduced accuracy (adaptive CG): series truncated to `order`, Clenshaw sweeps in fp32 if f32
+static int apply_A_reduced(ov_ctx* ctx, const double2* in, double2* tmp, double2* out, int order, bool f32) {
+    if (order >= ctx->order && !f32) return apply_A(ctx, in, tmp, out);
+    OV_TRY(apply_dov_reduced(ctx, 0.0, in, tmp, order, f32));
+    OV_TRY(launch_gamma5(ctx, tmp, tmp));
+    OV_TRY(apply_dov_reduced(ctx, 0.0, tmp, out, order, f32));
+    return launch_gamma5(ctx, out, out);
+}
+
+// d[n'] = max over x in [x_lo, 1] of sqrt(x) |P_n(x) - P_n'(x)|: how far the series truncated at n' is from the full
+// polynomial, as an operator on the part of the spectrum the polynomial acts on (host, a few hundred grid points)
+static std::vector<double> truncation_table(const std::vector<double>& c, double eps, double x_lo) {
+    const int n = (int)c.size() - 1, G = 600;
+    std::vector<double> d(n + 1, 0.0);
+    for (int g = 0; g < G; g++) {
+        const double u = (double)g / (G - 1);
+        const double x = (g % 2) ? x_lo * std::pow(1.0 / x_lo, u) : x_lo + (1.0 - x_lo) * u;   // log and linear grids
+        const double z = (2.0 * x - 1.0 - eps) / (1.0 - eps), sx = std::sqrt(x);
+        std::vector<double> T(n + 1);
+        T[0] = 1.0;
+        if (n >= 1) T[1] = z;
+        for (int j = 2; j <= n; j++) T[j] = 2.0 * z * T[j - 1] - T[j - 2];
+        double tail = 0.0;
+        for (int j = n; j >= 1; j--) {
+            tail += c[j] * T[j];
+            d[j - 1] = std::max(d[j - 1], sx * std::fabs(tail));
+        }
+    }
+    return d;
+}
+
 }  // namespace ov
 
 using namespace ov;
@@ -29,6 +60,7 @@ extern "C" int ov_multishift_cg(ov_ctx* ctx, const double* masses_host, int nmas
         return fail(ctx, OV_EINVAL, "bad argument to ov_multishift_cg");
     if (ctx->order < 0) return fail(ctx, OV_ESTATE, "ov_set_polynomial has not been called");
     const size_t n = spinor_elems(ctx), bytes = n * sizeof(double2);
+    ctx->cg_orders.clear();
     const double2* b = (const double2*)b_;
     double2* x = (double2*)x_;
 
@@ -66,6 +98,22 @@ extern "C" int ov_multishift_cg(ov_ctx* ctx, const double* masses_host, int nmas
         if (relres_out) for (int i = 0; i < nmass; i++) relres_out[i] = 0.0;
         return OV_OK;
     }
+    // adaptive accuracy (ov_set_cg_adaptive): the application of A at iteration j may be off by eta_j ~ tol |b| / |r_j|
+    std::vector<double> trunc;
+    if (ctx->cg_adaptive) {
+        double x_lo = ctx->eps;
+        if (ctx->k > 0) {
+            double lmax = 0.0;
+            for (double l : ctx->lambda) lmax = std::max(lmax, std::fabs(l));
+            x_lo = std::max(ctx->eps, 0.96 * lmax * lmax);
+        }
+        trunc = truncation_table(ctx->coef, ctx->eps, x_lo);
+    }
+    // relative error of an fp32 Clenshaw sweep: unit roundoff 6e-8 amplified by sum |c_j| (measured at 24^3x64, order
+    // 300, sum |c_j| ~ 100: 1.5e-6)
+    double csum = 0.0;
+    for (double cj : ctx->coef) csum += std::fabs(cj);
+    const double f32_floor = 6e-8 * csum;
     std::vector<double> zeta(nmass, 1.0), zeta_old(nmass, 1.0), zeta_new(nmass);
     std::vector<char> active(nmass, 1);
     double a_old = 1.0, beta_old = 0.0;
@@ -73,7 +121,15 @@ extern "C" int ov_multishift_cg(ov_ctx* ctx, const double* masses_host, int nmas
     bool converged = false;
     while (it < maxiter) {
         // q = (A + s0) p_0   (position 0 = smallest shift)
-        OV_TRY(apply_A(ctx, p[0], tmp, q));
+        int order = ctx->order;
+        bool f32 = false;
+        if (ctx->cg_adaptive) {
+            const double eta = std::min(0.1, 0.1 * tol * bnorm / std::sqrt(rr));   // allowed relative error of A p
+            while (order > 1 && 4.0 * trunc[order - 1] <= eta) order--;
+            f32 = ctx->cg_adaptive >= 2 && 4.0 * f32_floor <= eta;
+        }
+        OV_TRY(apply_A_reduced(ctx, p[0], tmp, q, order, f32));
+        if (ctx->cg_adaptive) { ctx->cg_orders.push_back(f32 ? -order : order); }
         if (s0 != 0.0) OV_TRY(launch_axpy(ctx, make_double2(s0, 0.0), p[0], q));
         double2 pq;
         OV_TRY(dot_host(ctx, p[0], q, &pq));

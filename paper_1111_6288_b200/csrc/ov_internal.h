@@ -41,16 +41,20 @@ struct Lattice {
 // Epilogue of the Wilson kernel:  out = s * G (in - kappa * hop(in)) + a1*A1 + a2*A2 + a3*A3
 //   G = gamma5 (g5 = 1) or the identity (g5 = 0);  hop_only: out = hop(in)  (no diagonal term, no axpy)
 // A1..A3 are optional ABI spinors read at the output site only, so `out` may alias any of them.
-struct Epilogue {
+// C = double2 (fp64, the product path) or float2 (the reduced-precision tail of the adaptive CG).
+template <typename C>
+struct EpilogueT {
     double s = 1.0;
     int g5 = 1;
     int hop_only = 0;
-    const double2* A1 = nullptr;
-    const double2* A2 = nullptr;
-    const double2* A3 = nullptr;
+    const C* A1 = nullptr;
+    const C* A2 = nullptr;
+    const C* A3 = nullptr;
     double a1 = 0.0, a2 = 0.0, a3 = 0.0;
     int a_g5 = 0;  // bit k-1 set: operand A_k enters as gamma5 A_k
 };
+using Epilogue = EpilogueT<double2>;
+using EpilogueF = EpilogueT<float2>;
 
 }  // namespace ov
 
@@ -60,7 +64,10 @@ struct ov_ctx {
     int recon = 18;
     cudaStream_t stream = nullptr;
     double2* gauge = nullptr;  // see gauge_index()
+    float2* gauge_f = nullptr; // fp32 copy of the links, same layout (made on first use by the adaptive CG)
     int dslash_variant = 0;
+    std::vector<int> cg_orders;  // order used at each iteration of the last adaptive CG (negative: fp32 sweep)
+    int cg_adaptive = 0;  // ov_set_cg_adaptive: 0 off, 1 reduced orders, 2 reduced orders + fp32 sweeps
     int flip = 0;  // block order of the next Wilson launch (alternates)
     bool blocked = false;  // layout of spinors and links (see spinor_base)
     long long launches = 0;
@@ -81,6 +88,7 @@ struct ov_ctx {
 
     // workspaces
     double2* ws[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    float2* wsf[4] = {nullptr, nullptr, nullptr, nullptr};  // fp32 Clenshaw vectors
     double2* d_partial = nullptr;  // reduction partials
     size_t partial_cap = 0;        // in double2
     double2* d_result = nullptr;   // reduced results (device)
@@ -127,6 +135,7 @@ int launch_pack(ov_ctx* ctx, const double2* canonical, double2* abi);
 int launch_unpack(ov_ctx* ctx, const double2* abi, double2* canonical);
 int launch_wilson(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep);
 int launch_wilson_gather(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep);
+int launch_wilson_gather_f32(ov_ctx* ctx, const float2* in, float2* out, const EpilogueF& ep);  // needs ctx->gauge_f
 int launch_wilson_tiled(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep);
 bool tiled_supported(const ov_ctx* ctx);
 // host-side dense Hermitian eigensolver (cyclic complex Jacobi): A (n x n, row-major complex, destroyed),
@@ -159,6 +168,13 @@ struct MultiAxpyOuts {
 int launch_multi_axpy(ov_ctx* ctx, const double2* xs, size_t stride, int nvec, int J, const double2* C_dev,
                       const double2* base, const MultiAxpyOuts& o);
 
+// fp32 helpers of the adaptive CG (blas.cu)
+int launch_scale_to_f32(ov_ctx* ctx, double a, const double2* x, float2* y);   // y = (float)(a x)
+int launch_combine_from_f32(ov_ctx* ctx, const float2* r, double a1, const double2* A1, double a2, const double2* A2,
+                            int a2_g5, double2* out);                          // out = r + a1 A1 + a2 [gamma5] A2
+int ensure_gauge_f32(ov_ctx* ctx);
+int workspace_f32(ov_ctx* ctx, int i, float2** out);
+
 // projector: c = V^+ x (left in ctx->d_result[0..k)); perp = x - V c; low = V (sgn o c)
 int project(ov_ctx* ctx, const double2* x, double2* perp, double2* low);
 
@@ -175,5 +191,6 @@ struct Span {
 int sign_poly(ov_ctx* ctx, const double2* x, double2* out, const Epilogue& fin);
 int apply_sign(ov_ctx* ctx, const double2* in, double2* out);
 int apply_dov(ov_ctx* ctx, double mass, const double2* in, double2* out);
+int apply_dov_reduced(ov_ctx* ctx, double mass, const double2* in, double2* out, int order, bool f32);
 
 }  // namespace ov

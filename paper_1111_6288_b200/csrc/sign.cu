@@ -36,50 +36,96 @@ int project(ov_ctx* ctx, const double2* x, double2* perp, double2* low) {
     return launch_multi_axpy(ctx, ctx->Vlow, stride, ctx->k, 2, ctx->d_coef, x, o);
 }
 
-// out = fin.s * G [Q P(Q^2) x]-ish: the last Wilson launch (result = Q y) carries `fin`:
-//   out = (fin.s / norm) * G (y - kappa hop y) + fin.a1 A1 + fin.a2 A2 + fin.a3 A3
+// Wilson launch by precision
+static int wilson_t(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep) { return launch_wilson(ctx, in, out, ep); }
+static int wilson_t(ov_ctx* ctx, const float2* in, float2* out, const EpilogueF& ep) { return launch_wilson_gather_f32(ctx, in, out, ep); }
+
+// Clenshaw sweep in precision C over the first n+1 coefficients c[0..n] (a truncation of the caller's series when
+// n < ctx->order: the adaptive CG's reduced orders).  b1 must hold c[n]*x on entry; b1, b2, t are scratch.
+//   out = (fin.s / norm) * G (y - kappa hop y) + fin.a1 A1 + fin.a2 A2 + fin.a3 A3,   y = P_n(Q^2) x
 // with fin.g5 = 1 -> G = gamma5 (plain sign), fin.g5 = 0 -> G = 1 (gamma5 * sign, for D_ov).
+template <typename C>
+static int clenshaw_t(ov_ctx* ctx, const double* c, int n, const C* x, C* out, const EpilogueT<C>& fin, C* b1, C* b2, C* t) {
+    const double eps = ctx->eps, inv = 1.0 / ctx->norm;
+    const double alpha = 4.0 / (1.0 - eps), beta = 2.0 * (1.0 + eps) / (1.0 - eps);
+    Span span(ctx, 0);  // every launch in here is the Wilson kernel
+    const C* y = b1;
+    bool b2_valid = false;
+    for (int j = n - 1; j >= 0; j--) {
+        EpilogueT<C> e1;  // t = Q b1
+        e1.s = inv;
+        e1.g5 = 1;
+        OV_TRY(wilson_t(ctx, b1, t, e1));
+        EpilogueT<C> e2;  // b2 <- f*(alpha Q t - beta b1) + c_j x - b2 ; f = 1 (j >= 1) or 1/2 (j = 0)
+        const double f = (j == 0) ? 0.5 : 1.0;
+        e2.s = f * alpha * inv;
+        e2.g5 = 1;
+        e2.A1 = x;  e2.a1 = c[j];
+        e2.A2 = b1; e2.a2 = -f * beta;
+        if (b2_valid) { e2.A3 = b2; e2.a3 = -1.0; }
+        OV_TRY(wilson_t(ctx, t, b2, e2));
+        b2_valid = true;
+        C* tmp = b1; b1 = b2; b2 = tmp;
+        y = b1;  // after the j = 0 step b1 holds y
+    }
+    EpilogueT<C> ef = fin;
+    ef.s = fin.s * inv;
+    ef.hop_only = 0;
+    return wilson_t(ctx, y, out, ef);
+}
+
 int sign_poly(ov_ctx* ctx, const double2* x, double2* out, const Epilogue& fin) {
     if (ctx->order < 0) return fail(ctx, OV_ESTATE, "ov_set_polynomial has not been called");
     const int n = ctx->order;
-    const double* c = ctx->coef.data();
-    const double eps = ctx->eps, inv = 1.0 / ctx->norm;
-    const double alpha = 4.0 / (1.0 - eps), beta = 2.0 * (1.0 + eps) / (1.0 - eps);
     double2 *b1, *b2, *t;
     OV_TRY(workspace(ctx, 0, &b1));
     OV_TRY(workspace(ctx, 1, &b2));
     OV_TRY(workspace(ctx, 2, &t));
+    OV_TRY(launch_axpby(ctx, ctx->coef[n], x, 0.0, nullptr, b1));   // b_n = c_n x  (b_{n+1} = b_{n+2} = 0)
+    return clenshaw_t<double2>(ctx, ctx->coef.data(), n, x, out, fin, b1, b2, t);
+}
 
-    // b_n = c_n x  (b_{n+1} = b_{n+2} = 0)
-    OV_TRY(launch_axpby(ctx, c[n], x, 0.0, nullptr, b1));
-    Span span(ctx, 0);  // from here on every launch is the Wilson kernel
-    const double2* y = nullptr;
-    if (n == 0) {
-        y = b1;
-    } else {
-        bool b2_valid = false;
-        for (int j = n - 1; j >= 0; j--) {
-            Epilogue e1;  // t = Q b1
-            e1.s = inv;
-            e1.g5 = 1;
-            OV_TRY(launch_wilson(ctx, b1, t, e1));
-            Epilogue e2;  // b2 <- f*(alpha Q t - beta b1) + c_j x - b2 ; f = 1 (j >= 1) or 1/2 (j = 0)
-            const double f = (j == 0) ? 0.5 : 1.0;
-            e2.s = f * alpha * inv;
-            e2.g5 = 1;
-            e2.A1 = x;  e2.a1 = c[j];
-            e2.A2 = b1; e2.a2 = -f * beta;
-            if (b2_valid) { e2.A3 = b2; e2.a3 = -1.0; }
-            OV_TRY(launch_wilson(ctx, t, b2, e2));
-            b2_valid = true;
-            double2* tmp = b1; b1 = b2; b2 = tmp;
-        }
-        y = b1;  // after the j = 0 step b1 holds y
+// D_ov(m) in at reduced accuracy (the adaptive CG): polynomial truncated to order n <= ctx->order and,
+// if f32, the Clenshaw sweep in single precision (projector and D_ov assembly stay fp64).
+int apply_dov_reduced(ov_ctx* ctx, double mass, const double2* in, double2* out, int n, bool f32) {
+    if (ctx->order < 0) return fail(ctx, OV_ESTATE, "ov_set_polynomial has not been called");
+    if (n < 0 || n > ctx->order) return fail(ctx, OV_EINVAL, "reduced order out of range");
+    const double2* perp = in;
+    double2* low = nullptr;
+    if (ctx->k > 0) {
+        double2* p;
+        OV_TRY(workspace(ctx, 3, &p));
+        OV_TRY(workspace(ctx, 4, &low));
+        OV_TRY(project(ctx, in, p, low));
+        perp = p;
     }
-    Epilogue ef = fin;
-    ef.s = fin.s * inv;
-    ef.hop_only = 0;
-    return launch_wilson(ctx, y, out, ef);
+    const double sm = 1.0 - 0.5 * mass, sp = 1.0 + 0.5 * mass;
+    if (!f32) {
+        double2 *b1, *b2, *t;
+        OV_TRY(workspace(ctx, 0, &b1));
+        OV_TRY(workspace(ctx, 1, &b2));
+        OV_TRY(workspace(ctx, 2, &t));
+        OV_TRY(launch_axpby(ctx, ctx->coef[n], perp, 0.0, nullptr, b1));
+        Epilogue fin;
+        fin.s = sm; fin.g5 = 0;
+        fin.A1 = in; fin.a1 = sp;
+        if (low) { fin.A2 = low; fin.a2 = sm; fin.a_g5 = 2; }
+        return clenshaw_t<double2>(ctx, ctx->coef.data(), n, perp, out, fin, b1, b2, t);
+    }
+    OV_TRY(ensure_gauge_f32(ctx));
+    float2 *xf, *b1, *b2, *t;
+    OV_TRY(workspace_f32(ctx, 0, &xf));
+    OV_TRY(workspace_f32(ctx, 1, &b1));
+    OV_TRY(workspace_f32(ctx, 2, &b2));
+    OV_TRY(workspace_f32(ctx, 3, &t));
+    OV_TRY(launch_scale_to_f32(ctx, 1.0, perp, xf));
+    OV_TRY(launch_scale_to_f32(ctx, ctx->coef[n], perp, b1));
+    EpilogueF fin;
+    fin.s = sm; fin.g5 = 0;
+    // the fp32 result r = (1-m/2) D_w y / norm lands in t's partner buffer; b2 or b1 may hold y, so use xf's slot last:
+    float2* r = (n % 2 == 0) ? b2 : b1;   // after n swaps y sits in b1 (n even) or b2 (n odd): write to the other one
+    OV_TRY(clenshaw_t<float2>(ctx, ctx->coef.data(), n, xf, r, fin, b1, b2, t));
+    return launch_combine_from_f32(ctx, r, sp, in, sm, low, 1, out);
 }
 
 int apply_sign(ov_ctx* ctx, const double2* in, double2* out) {

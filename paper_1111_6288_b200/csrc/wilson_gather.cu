@@ -6,8 +6,9 @@
 //   hop(in)(x) = sum_mu [ s+ (1-gamma_mu) U_mu(x) in(x+mu) + s- (1+gamma_mu) U_mu(x-mu)^+ in(x-mu) ]
 //
 // Layouts (ov_internal.h: spinor_base / gauge_index; blocked when V % 32 == 0, planes otherwise), NE = 9 link entries
-// (recon 18) or 6 (recon 12).  Either way a warp reads 32 consecutive double2 (512 B) per component or link entry:
-// fully coalesced LDG.128.
+// (recon 18) or 6 (recon 12).  Either way a warp reads 32 consecutive complex values (512 B in fp64: LDG.128; 256 B in fp32: LDG.64) per
+// component or link entry, fully coalesced.  The kernel is a template on the complex type: double2 is the product path,
+// float2 serves the reduced-precision tail of the adaptive CG.
 // Successive launches walk the lattice in opposite block order (GatherArgs::reverse): the spinor one launch wrote last
 // is what the next launch reads first, while it is still in the 126 MB L2.
 #include "ov_internal.h"
@@ -15,39 +16,41 @@
 
 namespace ov {
 
+template <typename C>
 struct GatherArgs {
-    const double2* gauge;
-    const double2* in;
-    double2* out;
+    const C* gauge;
+    const C* in;
+    C* out;
     int X, Y, Z, T;
     long long V;
     double kappa;
     int reverse;
-    Epilogue ep;
+    EpilogueT<C> ep;
 };
 
-// 64-thread blocks at <= 168 registers: 6 blocks = 12 warps per SM.  Measured at 24^3x64 (profiles/): 128 threads with
-// no register cap ran at 8 warps/SM and 215 us per apply, this shape at 166 us.
-constexpr int kGatherThreads = 64;
-constexpr int kGatherMinBlocks = 6;
+// fp64: 64-thread blocks at <= 168 registers: 6 blocks = 12 warps per SM.  Measured at 24^3x64 (profiles/): 128 threads
+// with no register cap ran at 8 warps/SM and 215 us per apply, this shape at 166 us.
+// fp32: half the registers per value: 128-thread blocks at <= 128 registers, 16 warps per SM.
+template <typename C> struct GatherShape;
+template <> struct GatherShape<double2> { static constexpr int threads = 64, min_blocks = 6; };
+template <> struct GatherShape<float2> { static constexpr int threads = 128, min_blocks = 4; };
 
-template <int RECON, bool BL>
-__device__ __forceinline__ void load_link(const double2* __restrict__ gauge, long long V, int mu,
-                                          long long site, double2* __restrict__ u) {
+template <int RECON, bool BL, typename C>
+__device__ __forceinline__ void load_link(const C* __restrict__ gauge, long long V, int mu, long long site,
+                                          C* __restrict__ u) {
     constexpr int NE = RECON / 2;
-    const double2* p = gauge + gauge_index<NE, BL>(V, mu, 0, site);
+    const C* p = gauge + gauge_index<NE, BL>(V, mu, 0, site);
     const long long es = BL ? 32 : V;  // stride between entries
 #pragma unroll
     for (int e = 0; e < NE; e++) u[e] = __ldg(p + (long long)e * es);
     if (RECON == 12) su3_row2(u);
 }
 
-template <int MU, int SIGMA, int RECON, bool BL>
-__device__ __forceinline__ void hop(double2* __restrict__ acc, const GatherArgs& a, long long nsite,
-                                    long long lsite, double ph) {
-    double2 psi[12], h[6], g[6], u[9];
-#pragma unroll
-    const double2* pn = a.in + spinor_base<BL>(nsite);
+template <int MU, int SIGMA, int RECON, bool BL, typename C>
+__device__ __forceinline__ void hop(C* __restrict__ acc, const GatherArgs<C>& a, long long nsite, long long lsite,
+                                    real_t<C> ph) {
+    C psi[12], h[6], g[6], u[9];
+    const C* pn = a.in + spinor_base<BL>(nsite);
     const long long cs = spinor_stride<BL>(a.V);
 #pragma unroll
     for (int c = 0; c < 12; c++) psi[c] = __ldg(pn + c * cs);
@@ -58,8 +61,10 @@ __device__ __forceinline__ void hop(double2* __restrict__ acc, const GatherArgs&
 }
 
 // NA: number of epilogue operands A1..A_NA (always filled in order); NA = -1: hop only
-template <int RECON, int NA, bool BL>
-__global__ void __launch_bounds__(kGatherThreads, kGatherMinBlocks) wilson_gather_kernel(const GatherArgs a) {
+template <typename C, int RECON, int NA, bool BL>
+__global__ void __launch_bounds__(GatherShape<C>::threads, GatherShape<C>::min_blocks)
+wilson_gather_kernel(const GatherArgs<C> a) {
+    using R = real_t<C>;
     const unsigned blk = a.reverse ? gridDim.x - 1 - blockIdx.x : blockIdx.x;
     const long long i = (long long)blk * blockDim.x + threadIdx.x;
     if (i >= a.V) return;
@@ -70,52 +75,51 @@ __global__ void __launch_bounds__(kGatherThreads, kGatherMinBlocks) wilson_gathe
     const int t = (int)(r / a.Z);
     const long long sX = 1, sY = a.X, sZ = (long long)a.X * a.Y, sT = (long long)a.X * a.Y * a.Z;
 
-
-    double2 acc[12];
+    C acc[12];
 #pragma unroll
-    for (int c = 0; c < 12; c++) acc[c] = make_double2(0.0, 0.0);
+    for (int c = 0; c < 12; c++) acc[c] = cmake<C>(0, 0);
 
     {
         const long long ip = (x + 1 == a.X) ? i - (a.X - 1) * sX : i + sX;
         const long long im = (x == 0) ? i + (a.X - 1) * sX : i - sX;
-        hop<0, -1, RECON, BL>(acc, a, ip, i, 1.0);
-        hop<0, +1, RECON, BL>(acc, a, im, im, 1.0);
+        hop<0, -1, RECON, BL>(acc, a, ip, i, (R)1);
+        hop<0, +1, RECON, BL>(acc, a, im, im, (R)1);
     }
     {
         const long long ip = (y + 1 == a.Y) ? i - (a.Y - 1) * sY : i + sY;
         const long long im = (y == 0) ? i + (a.Y - 1) * sY : i - sY;
-        hop<1, -1, RECON, BL>(acc, a, ip, i, 1.0);
-        hop<1, +1, RECON, BL>(acc, a, im, im, 1.0);
+        hop<1, -1, RECON, BL>(acc, a, ip, i, (R)1);
+        hop<1, +1, RECON, BL>(acc, a, im, im, (R)1);
     }
     {
         const long long ip = (z + 1 == a.Z) ? i - (a.Z - 1) * sZ : i + sZ;
         const long long im = (z == 0) ? i + (a.Z - 1) * sZ : i - sZ;
-        hop<2, -1, RECON, BL>(acc, a, ip, i, 1.0);
-        hop<2, +1, RECON, BL>(acc, a, im, im, 1.0);
+        hop<2, -1, RECON, BL>(acc, a, ip, i, (R)1);
+        hop<2, +1, RECON, BL>(acc, a, im, im, (R)1);
     }
     {
         const bool wp = (t + 1 == a.T), wm = (t == 0);
         const long long ip = wp ? i - (a.T - 1) * sT : i + sT;
         const long long im = wm ? i + (a.T - 1) * sT : i - sT;
-        hop<3, -1, RECON, BL>(acc, a, ip, i, wp ? -1.0 : 1.0);  // antiperiodic in time
-        hop<3, +1, RECON, BL>(acc, a, im, im, wm ? -1.0 : 1.0);
+        hop<3, -1, RECON, BL>(acc, a, ip, i, wp ? (R)-1 : (R)1);  // antiperiodic in time
+        hop<3, +1, RECON, BL>(acc, a, im, im, wm ? (R)-1 : (R)1);
     }
 
-    const Epilogue& ep = a.ep;
+    const EpilogueT<C>& ep = a.ep;
     const long long ib = spinor_base<BL>(i), cs = spinor_stride<BL>(a.V);
     if (NA < 0) {
 #pragma unroll
         for (int c = 0; c < 12; c++) a.out[ib + c * cs] = acc[c];
         return;
     }
-    const double slo = ep.g5 ? -ep.s : ep.s;
+    const R s_up = (R)ep.s, s_lo = (R)(ep.g5 ? -ep.s : ep.s), kappa = (R)a.kappa;
     // `out` may alias an operand (the Clenshaw step writes b_j over b_{j+2}), so the compiler must keep every operand
     // load behind the previous store: done component by component that is 12 dependent memory round trips.  Load a
     // chunk of components of every operand first (all loads in flight at once), then combine and store the chunk.
     constexpr int CH = 4;
 #pragma unroll
     for (int c0 = 0; c0 < 12; c0 += CH) {
-        double2 own[CH], w1[CH], w2[CH], w3[CH];
+        C own[CH], w1[CH], w2[CH], w3[CH];
 #pragma unroll
         for (int k = 0; k < CH; k++) {
             const long long e = ib + (c0 + k) * cs;
@@ -128,19 +132,20 @@ __global__ void __launch_bounds__(kGatherThreads, kGatherMinBlocks) wilson_gathe
         for (int k = 0; k < CH; k++) {
             const int c = c0 + k;
             const bool lo = (c >= 6);
-            const double sc = lo ? slo : ep.s;
-            double2 v = make_double2(sc * fma(-a.kappa, acc[c].x, own[k].x), sc * fma(-a.kappa, acc[c].y, own[k].y));
-            if (NA >= 1) { const double f = (lo && (ep.a_g5 & 1)) ? -ep.a1 : ep.a1; v.x = fma(f, w1[k].x, v.x); v.y = fma(f, w1[k].y, v.y); }
-            if (NA >= 2) { const double f = (lo && (ep.a_g5 & 2)) ? -ep.a2 : ep.a2; v.x = fma(f, w2[k].x, v.x); v.y = fma(f, w2[k].y, v.y); }
-            if (NA >= 3) { const double f = (lo && (ep.a_g5 & 4)) ? -ep.a3 : ep.a3; v.x = fma(f, w3[k].x, v.x); v.y = fma(f, w3[k].y, v.y); }
+            const R sc = lo ? s_lo : s_up;
+            C v = cmake<C>(sc * fma(-kappa, acc[c].x, own[k].x), sc * fma(-kappa, acc[c].y, own[k].y));
+            if (NA >= 1) { const R f = (R)((lo && (ep.a_g5 & 1)) ? -ep.a1 : ep.a1); v.x = fma(f, w1[k].x, v.x); v.y = fma(f, w1[k].y, v.y); }
+            if (NA >= 2) { const R f = (R)((lo && (ep.a_g5 & 2)) ? -ep.a2 : ep.a2); v.x = fma(f, w2[k].x, v.x); v.y = fma(f, w2[k].y, v.y); }
+            if (NA >= 3) { const R f = (R)((lo && (ep.a_g5 & 4)) ? -ep.a3 : ep.a3); v.x = fma(f, w3[k].x, v.x); v.y = fma(f, w3[k].y, v.y); }
             a.out[ib + c * cs] = v;
         }
     }
 }
 
-int launch_wilson_gather(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep) {
-    GatherArgs a;
-    a.gauge = ctx->gauge;
+template <typename C>
+static int launch_gather_t(ov_ctx* ctx, const C* gauge, const C* in, C* out, const EpilogueT<C>& ep) {
+    GatherArgs<C> a;
+    a.gauge = gauge;
     a.in = in;
     a.out = out;
     a.X = ctx->lat.X; a.Y = ctx->lat.Y; a.Z = ctx->lat.Z; a.T = ctx->lat.T;
@@ -153,14 +158,14 @@ int launch_wilson_gather(ov_ctx* ctx, const double2* in, double2* out, const Epi
     a.reverse = ctx->flip;
     ctx->flip ^= 1;
 #endif
-    const int threads = kGatherThreads;
+    const int threads = GatherShape<C>::threads;
     const unsigned blocks = (unsigned)((a.V + threads - 1) / threads);
     const int na = ep.hop_only ? -1 : (ep.A3 ? 3 : ep.A2 ? 2 : ep.A1 ? 1 : 0);
     if ((ep.A3 && !ep.A2) || (ep.A2 && !ep.A1)) return fail(ctx, OV_EINVAL, "epilogue operands must be filled in order");
-#define OV_GATHER(R, N)                                                                   \
-    do {                                                                                  \
-        if (ctx->blocked) wilson_gather_kernel<R, N, true><<<blocks, threads, 0, ctx->stream>>>(a);  \
-        else wilson_gather_kernel<R, N, false><<<blocks, threads, 0, ctx->stream>>>(a);   \
+#define OV_GATHER(R, N)                                                                                  \
+    do {                                                                                                 \
+        if (ctx->blocked) wilson_gather_kernel<C, R, N, true><<<blocks, threads, 0, ctx->stream>>>(a);   \
+        else wilson_gather_kernel<C, R, N, false><<<blocks, threads, 0, ctx->stream>>>(a);               \
     } while (0)
 #define OV_GATHER_NA(R)                                 \
     switch (na) {                                       \
@@ -176,6 +181,14 @@ int launch_wilson_gather(ov_ctx* ctx, const double2* in, double2* out, const Epi
     ctx->launches++;
     OV_CUDA(ctx, cudaGetLastError());
     return OV_OK;
+}
+
+int launch_wilson_gather(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep) {
+    return launch_gather_t<double2>(ctx, ctx->gauge, in, out, ep);
+}
+int launch_wilson_gather_f32(ov_ctx* ctx, const float2* in, float2* out, const EpilogueF& ep) {
+    if (!ctx->gauge_f) return fail(ctx, OV_ESTATE, "fp32 links have not been made");
+    return launch_gather_t<float2>(ctx, ctx->gauge_f, in, out, ep);
 }
 
 }  // namespace ov

@@ -8,39 +8,40 @@
 
 namespace ov {
 
-__device__ __forceinline__ double2 cadd(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ double2 csub(double2 a, double2 b) { return make_double2(a.x - b.x, a.y - b.y); }
+// complex types: double2 (the product path, fp64) and float2 (the reduced-precision tail of the adaptive CG)
+template <typename C> struct real_of;
+template <> struct real_of<double2> { using type = double; };
+template <> struct real_of<float2> { using type = float; };
+template <typename C> using real_t = typename real_of<C>::type;
+template <typename C> __device__ __forceinline__ C cmake(real_t<C> x, real_t<C> y) { C c; c.x = x; c.y = y; return c; }
+
+template <typename C> __device__ __forceinline__ C cadd(C a, C b) { return cmake<C>(a.x + b.x, a.y + b.y); }
+template <typename C> __device__ __forceinline__ C csub(C a, C b) { return cmake<C>(a.x - b.x, a.y - b.y); }
 // a + i*s*b
-__device__ __forceinline__ double2 caddi(double2 a, double2 b, double s) {
-    return make_double2(a.x - s * b.y, a.y + s * b.x);
-}
+template <typename C> __device__ __forceinline__ C caddi(C a, C b, real_t<C> s) { return cmake<C>(a.x - s * b.y, a.y + s * b.x); }
 // a + s*b (s real)
-__device__ __forceinline__ double2 cadds(double2 a, double2 b, double s) {
-    return make_double2(a.x + s * b.x, a.y + s * b.y);
-}
+template <typename C> __device__ __forceinline__ C cadds(C a, C b, real_t<C> s) { return cmake<C>(a.x + s * b.x, a.y + s * b.y); }
 // acc += a*b
-__device__ __forceinline__ void cmadd(double2& acc, double2 a, double2 b) {
+template <typename C> __device__ __forceinline__ void cmadd(C& acc, C a, C b) {
     acc.x = fma(a.x, b.x, acc.x);
     acc.x = fma(-a.y, b.y, acc.x);
     acc.y = fma(a.x, b.y, acc.y);
     acc.y = fma(a.y, b.x, acc.y);
 }
 // acc += conj(a)*b
-__device__ __forceinline__ void cmaddc(double2& acc, double2 a, double2 b) {
+template <typename C> __device__ __forceinline__ void cmaddc(C& acc, C a, C b) {
     acc.x = fma(a.x, b.x, acc.x);
     acc.x = fma(a.y, b.y, acc.x);
     acc.y = fma(a.x, b.y, acc.y);
     acc.y = fma(-a.y, b.x, acc.y);
 }
-__device__ __forceinline__ double2 cmul(double2 a, double2 b) {
-    return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
-}
-__device__ __forceinline__ double2 cconj(double2 a) { return make_double2(a.x, -a.y); }
+template <typename C> __device__ __forceinline__ C cmul(C a, C b) { return cmake<C>(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+template <typename C> __device__ __forceinline__ C cconj(C a) { return cmake<C>(a.x, -a.y); }
 
 // h = upper half of (1 + SIGMA*gamma_MU) psi ; psi[3*spin + colour]
-template <int MU, int SIGMA>
-__device__ __forceinline__ void project(const double2* __restrict__ psi, double2* __restrict__ h) {
-    constexpr double s = (double)SIGMA;
+template <int MU, int SIGMA, typename C>
+__device__ __forceinline__ void project(const C* __restrict__ psi, C* __restrict__ h) {
+    constexpr real_t<C> s = (real_t<C>)SIGMA;
 #pragma unroll
     for (int c = 0; c < 3; c++) {
         if (MU == 0) {  // r0 = psi0 - i s psi3 ; r1 = psi1 - i s psi2
@@ -60,10 +61,9 @@ __device__ __forceinline__ void project(const double2* __restrict__ psi, double2
 }
 
 // acc += full (1 + SIGMA*gamma_MU)-spinor whose upper half is g (times the real factor ph = +-1)
-template <int MU, int SIGMA>
-__device__ __forceinline__ void reconstruct_add(double2* __restrict__ acc, const double2* __restrict__ g,
-                                                double ph) {
-    const double s = (double)SIGMA * ph;
+template <int MU, int SIGMA, typename C>
+__device__ __forceinline__ void reconstruct_add(C* __restrict__ acc, const C* __restrict__ g, real_t<C> ph) {
+    const real_t<C> s = (real_t<C>)SIGMA * ph;
 #pragma unroll
     for (int c = 0; c < 3; c++) {
         acc[c] = cadds(acc[c], g[c], ph);
@@ -85,21 +85,21 @@ __device__ __forceinline__ void reconstruct_add(double2* __restrict__ acc, const
 }
 
 // third row of an SU(3) matrix from the first two: row2 = conj(row0 x row1)
-__device__ __forceinline__ void su3_row2(double2* __restrict__ u) {
+template <typename C>
+__device__ __forceinline__ void su3_row2(C* __restrict__ u) {
     u[6] = cconj(csub(cmul(u[1], u[5]), cmul(u[2], u[4])));
     u[7] = cconj(csub(cmul(u[2], u[3]), cmul(u[0], u[5])));
     u[8] = cconj(csub(cmul(u[0], u[4]), cmul(u[1], u[3])));
 }
 
 // g = U h (DAG = false) or U^dagger h (DAG = true) on both spin components of a half-spinor
-template <bool DAG>
-__device__ __forceinline__ void su3_mul(const double2* __restrict__ u, const double2* __restrict__ h,
-                                        double2* __restrict__ g) {
+template <bool DAG, typename C>
+__device__ __forceinline__ void su3_mul(const C* __restrict__ u, const C* __restrict__ h, C* __restrict__ g) {
 #pragma unroll
     for (int sp = 0; sp < 2; sp++) {
 #pragma unroll
         for (int a = 0; a < 3; a++) {
-            double2 acc = make_double2(0.0, 0.0);
+            C acc = cmake<C>(0, 0);
 #pragma unroll
             for (int b = 0; b < 3; b++) {
                 if (DAG)

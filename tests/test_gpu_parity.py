@@ -247,3 +247,40 @@ def test_lanczos_4x4_vs_dense(ovp, cfg0):
         assert np.linalg.norm(r.ravel()) <= 1e-8
     G = Vh.reshape(k, -1).conj() @ Vh.reshape(k, -1).T
     assert np.max(np.abs(G - np.eye(k))) <= 1e-10
+
+
+# ------------------------------------------------------------------------------------------ adaptive CG
+def test_reduced_dov_vs_oracle(ovp, cfg0):
+    """The truncated series is the oracle's D_ov with the first n'+1 coefficients; the fp32 sweep agrees with the fp64
+    one to single-precision rounding (amplified by the Clenshaw recurrence)."""
+    c = cfg0
+    cfg = c["cfg"]
+    op, coef = setup_op(ovp, c)
+    dx = to_dev(op, c["x"])
+    for n_red in (cfg.order, 20, 7):
+        ref = oracle.dov(cfg.dims, cfg.kappa, c["U"], coef[:n_red + 1], cfg.eps, cfg.norm, c["V"], c["lam"], 0.1, c["x"])
+        assert rel(to_host(op, op.apply_dov_reduced(0.1, dx, n_red, False)), ref) <= TOL_DOV
+        assert rel(to_host(op, op.apply_dov_reduced(0.1, dx, n_red, True)), ref) <= 2e-5
+    assert rel(to_host(op, op.apply_dov_reduced(0.0, dx, cfg.order, False)), to_host(op, op.apply_dov(0.0, dx))) <= 1e-14
+
+
+@pytest.mark.parametrize("mode", [1, 2])
+def test_adaptive_multishift_cg(ovp, cfg0, mode):
+    c = cfg0
+    cfg = c["cfg"]
+    op, coef = setup_op(ovp, c)
+    masses = (0.1, 0.005, 0.04)
+    b = to_dev(op, c["x"])
+    x0, it0, res0, ok0 = op.multishift_cg(masses, b, tol=1e-8, maxiter=300)
+    op.set_cg_adaptive(mode)
+    x1, it1, res1, ok1 = op.multishift_cg(masses, b, tol=1e-8, maxiter=300)
+    orders = op.cg_orders()
+    op.set_cg_adaptive(0)
+    assert ok0 and ok1 and np.all(res1 <= 1e-8)          # true residuals, recomputed with the full fp64 operator
+    assert abs(it1 - it0) <= 2
+    assert len(orders) == it1 and abs(orders[0]) == cfg.order and min(abs(o) for o in orders) < cfg.order
+    if mode == 2:
+        assert any(o < 0 for o in orders)                 # some sweeps ran in fp32
+    g0, g1 = to_host(op, x0), to_host(op, x1)
+    for i in range(len(masses)):
+        assert rel(g1[i], g0[i]) <= 1e-6
