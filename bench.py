@@ -49,6 +49,7 @@ def parse_args():
     ap.add_argument("--lanczos-order", type=int, default=100, help="Chebyshev filter order (paper: 100)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cg", action="store_true")
     return ap.parse_args()
 
 
@@ -355,12 +356,29 @@ def run_b200(args):
     del a, b
     hw_gbs = (384.0 + 32.0 * args.recon) * V_sites * nhw / (ms_hw * 1e-3) / 1e9
 
+    # ---- multi-mass CG time-to-solution on the same lattice (north_star: reported beside the headline)
+    cg = None
+    if k > 0 and world == 1 and not args.no_cg:
+        masses = wl.CONFIGS[4].masses
+        bsrc = op.pack_spinor(torch.from_numpy(wl.point_source(cfg.dims)).cuda())
+        cg = {"masses": list(masses), "tol": 1e-8, "source": "point"}
+        for mode, name in ((0, "plain"), (2, "adaptive")):
+            op.set_cg_adaptive(mode)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            xs, iters, _, okc = op.multishift_cg(masses, bsrc, tol=1e-8, maxiter=200, true_residuals=False)
+            torch.cuda.synchronize()
+            cg[name] = {"seconds": time.perf_counter() - t0, "iterations": iters, "converged": bool(okc)}
+            if mode == 2:
+                cg[name]["orders"] = op.cg_orders()
+        op.set_cg_adaptive(0)
+        del xs, bsrc
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return 0
     return finish(args, cfg, order, k, V_sites, world, ms, value, launches, tim, e2e, hw_gbs, ms_hw / nhw,
-                  sampler, lanczos_s, resid, U, log)
+                  sampler, lanczos_s, resid, U, log, cg)
 
 
 class _Null:
@@ -389,7 +407,7 @@ def ncu_traffic():
 
 
 def finish(args, cfg, order, k, V_sites, world, ms, value, launches, tim, e2e, hw_gbs, hw_ms, sampler,
-           lanczos_s, resid, U, log):
+           lanczos_s, resid, U, log, cg=None):
     peak, peak_src = measured_peak()
     nsign = args.steps
     wl_launches = tim["wilson_launches"]
@@ -420,7 +438,7 @@ def finish(args, cfg, order, k, V_sites, world, ms, value, launches, tim, e2e, h
         "config": {"workload": workload_name(cfg, order, k), "recon": args.recon, "parallelism": f"replicas x{world}",
                    "l2": "inputs larger than L2 (gauge 510 MB + 17 GB of low modes stream every step)",
                    "low_modes": f"GPU Lanczos, max residual {resid:.1e}, {lanczos_s:.0f} s (untimed setup)" if k else "none"},
-        "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
+        "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu, "cg_time_to_solution": cg,
         "paper_context": "paper: ~30 CPU cores per GPU on unnamed 6 GB GPUs vs Cray XT-5 (PAPER.md:9) - context only",
     }
     print(json.dumps(line), flush=True)

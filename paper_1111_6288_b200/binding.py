@@ -268,14 +268,15 @@ class Overlap:
         return out.value
 
     # ---- consumers
-    def multishift_cg(self, masses, b, tol=1e-8, maxiter=1000):
+    def multishift_cg(self, masses, b, tol=1e-8, maxiter=1000, true_residuals=True):
+        """x[nmass], iterations, true relative residuals (None if not asked for), converged"""
         m, pm = _darr(masses)
         x = self.new_spinor(len(m))
         iters = ctypes.c_int()
-        res = np.empty(len(m))
+        res = np.empty(len(m)) if true_residuals else None
+        pres = res.ctypes.data_as(ctypes.POINTER(ctypes.c_double)) if true_residuals else None
         rc = self.lib.ov_multishift_cg(self._ctx, pm, ctypes.c_int(len(m)), _ptr(b), _ptr(x), ctypes.c_double(tol),
-                                       ctypes.c_int(maxiter), ctypes.byref(iters),
-                                       res.ctypes.data_as(ctypes.POINTER(ctypes.c_double)))
+                                       ctypes.c_int(maxiter), ctypes.byref(iters), pres)
         if rc not in (OV_OK, OV_ENOCONV):
             self._check(rc)
         return x, iters.value, res, rc == OV_OK
