@@ -356,6 +356,16 @@ def run_b200(args):
     del a, b
     hw_gbs = (384.0 + 32.0 * args.recon) * V_sites * nhw / (ms_hw * 1e-3) / 1e9
 
+    # ---- batched right-hand sides (reported separately, G17): 4 sources per Clenshaw sweep
+    batched = None
+    if not args.no_e2e and nsrc >= 4:
+        xb = torch.stack(dev_src[:4]).contiguous()
+        yb = torch.empty_like(xb)
+        ms_b = timed(lambda i: op.apply_dov(0.0, xb, yb), 1, 2)
+        batched = {"nrhs": 4, "value": aggregate_value(world, 2 * 4, ms_b), "unit": UNIT,
+                   "note": "ov_apply_dov(nrhs=4): every Wilson launch covers 4 right-hand sides"}
+        del xb, yb
+
     # ---- multi-mass CG time-to-solution on the same lattice (north_star: reported beside the headline)
     cg = None
     if k > 0 and world == 1 and not args.no_cg:
@@ -378,7 +388,7 @@ def run_b200(args):
             dist.destroy_process_group()
         return 0
     return finish(args, cfg, order, k, V_sites, world, ms, value, launches, tim, e2e, hw_gbs, ms_hw / nhw,
-                  sampler, lanczos_s, resid, U, log, cg)
+                  sampler, lanczos_s, resid, U, log, cg, batched)
 
 
 class _Null:
@@ -407,7 +417,7 @@ def ncu_traffic():
 
 
 def finish(args, cfg, order, k, V_sites, world, ms, value, launches, tim, e2e, hw_gbs, hw_ms, sampler,
-           lanczos_s, resid, U, log, cg=None):
+           lanczos_s, resid, U, log, cg=None, batched=None):
     peak, peak_src = measured_peak()
     nsign = args.steps
     wl_launches = tim["wilson_launches"]
@@ -438,7 +448,7 @@ def finish(args, cfg, order, k, V_sites, world, ms, value, launches, tim, e2e, h
         "config": {"workload": workload_name(cfg, order, k), "recon": args.recon, "parallelism": f"replicas x{world}",
                    "l2": "inputs larger than L2 (gauge 510 MB + 17 GB of low modes stream every step)",
                    "low_modes": f"GPU Lanczos, max residual {resid:.1e}, {lanczos_s:.0f} s (untimed setup)" if k else "none"},
-        "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu, "cg_time_to_solution": cg,
+        "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu, "cg_time_to_solution": cg, "batched": batched,
         "paper_context": "paper: ~30 CPU cores per GPU on unnamed 6 GB GPUs vs Cray XT-5 (PAPER.md:9) - context only",
     }
     print(json.dumps(line), flush=True)

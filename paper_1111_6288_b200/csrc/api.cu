@@ -140,6 +140,7 @@ void ov_destroy(ov_ctx* ctx) {
     for (auto& w : ctx->ws) cudaFree(w);
     for (auto& w : ctx->wsf) cudaFree(w);
     cudaFree(ctx->gauge_f);
+    cudaFree(ctx->wsb);
     cudaFree(ctx->d_partial);
     cudaFree(ctx->d_result);
     if (ctx->h_result) cudaFreeHost(ctx->h_result);
@@ -212,16 +213,16 @@ int ov_dslash(ov_ctx* ctx, const void* in, void* out, int nrhs) {
     const size_t n = spinor_elems(ctx);
     Epilogue ep;
     ep.hop_only = 1;
-    for (int r = 0; r < nrhs; r++) OV_TRY(launch_wilson(ctx, (const double2*)in + r * n, (double2*)out + r * n, ep));
-    return OV_OK;
+    (void)n;
+    return launch_wilson_batch(ctx, (const double2*)in, (double2*)out, ep, nrhs);
 }
 
 int ov_apply_hw(ov_ctx* ctx, const void* in, void* out, int nrhs) {
     OV_TRY(check_apply(ctx, in, out, nrhs));
     const size_t n = spinor_elems(ctx);
     Epilogue ep;  // s = 1, gamma5
-    for (int r = 0; r < nrhs; r++) OV_TRY(launch_wilson(ctx, (const double2*)in + r * n, (double2*)out + r * n, ep));
-    return OV_OK;
+    (void)n;
+    return launch_wilson_batch(ctx, (const double2*)in, (double2*)out, ep, nrhs);
 }
 
 }  // extern "C"

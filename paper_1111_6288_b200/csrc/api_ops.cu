@@ -100,14 +100,26 @@ int ov_project(ov_ctx* ctx, const void* in, void* perp, void* low, double* coef_
 int ov_apply_sign(ov_ctx* ctx, const void* in, void* out, int nrhs) {
     OV_TRY(check2(ctx, in, out, nrhs));
     const size_t n = spinor_elems(ctx);
-    for (int r = 0; r < nrhs; r++) OV_TRY(apply_sign(ctx, (const double2*)in + r * n, (double2*)out + r * n));
+    int r = 0;
+    for (; nrhs - r >= 2; ) {   // batches of up to kBatch right-hand sides share every Wilson launch
+        const int nb = nrhs - r >= kBatch ? kBatch : nrhs - r;
+        OV_TRY(apply_batch(ctx, true, 0.0, (const double2*)in + r * n, (double2*)out + r * n, nb));
+        r += nb;
+    }
+    for (; r < nrhs; r++) OV_TRY(apply_sign(ctx, (const double2*)in + r * n, (double2*)out + r * n));
     return OV_OK;
 }
 
 int ov_apply_dov(ov_ctx* ctx, double mass, const void* in, void* out, int nrhs) {
     OV_TRY(check2(ctx, in, out, nrhs));
     const size_t n = spinor_elems(ctx);
-    for (int r = 0; r < nrhs; r++) OV_TRY(apply_dov(ctx, mass, (const double2*)in + r * n, (double2*)out + r * n));
+    int r = 0;
+    for (; nrhs - r >= 2; ) {
+        const int nb = nrhs - r >= kBatch ? kBatch : nrhs - r;
+        OV_TRY(apply_batch(ctx, false, mass, (const double2*)in + r * n, (double2*)out + r * n, nb));
+        r += nb;
+    }
+    for (; r < nrhs; r++) OV_TRY(apply_dov(ctx, mass, (const double2*)in + r * n, (double2*)out + r * n));
     return OV_OK;
 }
 

@@ -142,8 +142,8 @@ int launch_axpy(ov_ctx* ctx, double2 a, const double2* x, double2* y) {
     OV_CUDA(ctx, cudaGetLastError());
     return OV_OK;
 }
-int launch_axpby(ov_ctx* ctx, double a, const double2* x, double b, const double2* y, double2* z) {
-    const long long n = (long long)spinor_elems(ctx);
+int launch_axpby(ov_ctx* ctx, double a, const double2* x, double b, const double2* y, double2* z, int nrhs) {
+    const long long n = (long long)spinor_elems(ctx) * nrhs;
     axpby_kernel<<<ew_blocks(n), kEwThreads, 0, ctx->stream>>>(a, x, b, y, z, n);
     ctx->launches++;
     OV_CUDA(ctx, cudaGetLastError());

@@ -89,6 +89,7 @@ struct ov_ctx {
     // workspaces
     double2* ws[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     float2* wsf[4] = {nullptr, nullptr, nullptr, nullptr};  // fp32 Clenshaw vectors
+    double2* wsb = nullptr;  // batched Clenshaw: 5 x kBatch spinors (b1, b2, t, x_perp, x_low)
     double2* d_partial = nullptr;  // reduction partials
     size_t partial_cap = 0;        // in double2
     double2* d_result = nullptr;   // reduced results (device)
@@ -135,6 +136,8 @@ int launch_pack(ov_ctx* ctx, const double2* canonical, double2* abi);
 int launch_unpack(ov_ctx* ctx, const double2* abi, double2* canonical);
 int launch_wilson(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep);
 int launch_wilson_gather(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep);
+// batched: nrhs consecutive ABI spinors (stride 12 V) in in/out and in every epilogue operand
+int launch_wilson_batch(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep, int nrhs);
 int launch_wilson_gather_f32(ov_ctx* ctx, const float2* in, float2* out, const EpilogueF& ep);  // needs ctx->gauge_f
 int launch_wilson_tiled(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep);
 bool tiled_supported(const ov_ctx* ctx);
@@ -144,7 +147,7 @@ void host_eigh(int n, std::vector<double2>& A, std::vector<double>& w, std::vect
 
 // BLAS-1 on ABI spinors (n = 12 V complex)
 int launch_axpy(ov_ctx* ctx, double2 a, const double2* x, double2* y);                     // y += a x
-int launch_axpby(ov_ctx* ctx, double a, const double2* x, double b, const double2* y, double2* z);  // z = a x + b y
+int launch_axpby(ov_ctx* ctx, double a, const double2* x, double b, const double2* y, double2* z, int nrhs = 1);  // z = a x + b y
 int launch_scale(ov_ctx* ctx, double a, double2* x);
 int launch_copy(ov_ctx* ctx, const double2* x, double2* y);
 int launch_zero(ov_ctx* ctx, double2* x);
@@ -191,6 +194,9 @@ struct Span {
 int sign_poly(ov_ctx* ctx, const double2* x, double2* out, const Epilogue& fin);
 int apply_sign(ov_ctx* ctx, const double2* in, double2* out);
 int apply_dov(ov_ctx* ctx, double mass, const double2* in, double2* out);
+// nb <= kBatch right-hand sides through one batched Clenshaw sweep (gamma5_out = false: D_ov(mass); true: sign)
+constexpr int kBatch = 4;
+int apply_batch(ov_ctx* ctx, bool sign_only, double mass, const double2* in, double2* out, int nb);
 int apply_dov_reduced(ov_ctx* ctx, double mass, const double2* in, double2* out, int order, bool f32);
 
 }  // namespace ov

@@ -37,15 +37,18 @@ int project(ov_ctx* ctx, const double2* x, double2* perp, double2* low) {
 }
 
 // Wilson launch by precision
-static int wilson_t(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep) { return launch_wilson(ctx, in, out, ep); }
-static int wilson_t(ov_ctx* ctx, const float2* in, float2* out, const EpilogueF& ep) { return launch_wilson_gather_f32(ctx, in, out, ep); }
+static int wilson_t(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep, int nb) {
+    return nb > 1 ? launch_wilson_batch(ctx, in, out, ep, nb) : launch_wilson(ctx, in, out, ep);
+}
+static int wilson_t(ov_ctx* ctx, const float2* in, float2* out, const EpilogueF& ep, int) { return launch_wilson_gather_f32(ctx, in, out, ep); }
 
 // Clenshaw sweep in precision C over the first n+1 coefficients c[0..n] (a truncation of the caller's series when
 // n < ctx->order: the adaptive CG's reduced orders).  b1 must hold c[n]*x on entry; b1, b2, t are scratch.
 //   out = (fin.s / norm) * G (y - kappa hop y) + fin.a1 A1 + fin.a2 A2 + fin.a3 A3,   y = P_n(Q^2) x
 // with fin.g5 = 1 -> G = gamma5 (plain sign), fin.g5 = 0 -> G = 1 (gamma5 * sign, for D_ov).
 template <typename C>
-static int clenshaw_t(ov_ctx* ctx, const double* c, int n, const C* x, C* out, const EpilogueT<C>& fin, C* b1, C* b2, C* t) {
+static int clenshaw_t(ov_ctx* ctx, const double* c, int n, const C* x, C* out, const EpilogueT<C>& fin, C* b1, C* b2, C* t,
+                      int nb = 1) {
     const double eps = ctx->eps, inv = 1.0 / ctx->norm;
     const double alpha = 4.0 / (1.0 - eps), beta = 2.0 * (1.0 + eps) / (1.0 - eps);
     Span span(ctx, 0);  // every launch in here is the Wilson kernel
@@ -55,7 +58,7 @@ static int clenshaw_t(ov_ctx* ctx, const double* c, int n, const C* x, C* out, c
         EpilogueT<C> e1;  // t = Q b1
         e1.s = inv;
         e1.g5 = 1;
-        OV_TRY(wilson_t(ctx, b1, t, e1));
+        OV_TRY(wilson_t(ctx, b1, t, e1, nb));
         EpilogueT<C> e2;  // b2 <- f*(alpha Q t - beta b1) + c_j x - b2 ; f = 1 (j >= 1) or 1/2 (j = 0)
         const double f = (j == 0) ? 0.5 : 1.0;
         e2.s = f * alpha * inv;
@@ -63,7 +66,7 @@ static int clenshaw_t(ov_ctx* ctx, const double* c, int n, const C* x, C* out, c
         e2.A1 = x;  e2.a1 = c[j];
         e2.A2 = b1; e2.a2 = -f * beta;
         if (b2_valid) { e2.A3 = b2; e2.a3 = -1.0; }
-        OV_TRY(wilson_t(ctx, t, b2, e2));
+        OV_TRY(wilson_t(ctx, t, b2, e2, nb));
         b2_valid = true;
         C* tmp = b1; b1 = b2; b2 = tmp;
         y = b1;  // after the j = 0 step b1 holds y
@@ -71,7 +74,7 @@ static int clenshaw_t(ov_ctx* ctx, const double* c, int n, const C* x, C* out, c
     EpilogueT<C> ef = fin;
     ef.s = fin.s * inv;
     ef.hop_only = 0;
-    return wilson_t(ctx, y, out, ef);
+    return wilson_t(ctx, y, out, ef, nb);
 }
 
 int sign_poly(ov_ctx* ctx, const double2* x, double2* out, const Epilogue& fin) {
@@ -83,6 +86,33 @@ int sign_poly(ov_ctx* ctx, const double2* x, double2* out, const Epilogue& fin) 
     OV_TRY(workspace(ctx, 2, &t));
     OV_TRY(launch_axpby(ctx, ctx->coef[n], x, 0.0, nullptr, b1));   // b_n = c_n x  (b_{n+1} = b_{n+2} = 0)
     return clenshaw_t<double2>(ctx, ctx->coef.data(), n, x, out, fin, b1, b2, t);
+}
+
+// nb right-hand sides at once: per-rhs projector, then ONE Clenshaw sweep whose every launch covers the whole batch
+// (the links are then read from HBM once per site block and shared through L2/L1 by the right-hand sides).
+int apply_batch(ov_ctx* ctx, bool sign_only, double mass, const double2* in, double2* out, int nb) {
+    if (ctx->order < 0) return fail(ctx, OV_ESTATE, "ov_set_polynomial has not been called");
+    if (nb < 1 || nb > kBatch) return fail(ctx, OV_EINVAL, "batch size out of range");
+    const size_t n = spinor_elems(ctx);
+    if (!ctx->wsb) OV_CUDA(ctx, cudaMalloc(&ctx->wsb, (size_t)5 * kBatch * n * sizeof(double2)));
+    double2 *b1 = ctx->wsb, *b2 = b1 + kBatch * n, *t = b2 + kBatch * n, *perp = t + kBatch * n, *low = perp + kBatch * n;
+    const double2* x = in;
+    if (ctx->k > 0) {
+        for (int r = 0; r < nb; r++) OV_TRY(project(ctx, in + r * n, perp + r * n, low + r * n));
+        x = perp;
+    }
+    const int order = ctx->order;
+    OV_TRY(launch_axpby(ctx, ctx->coef[order], x, 0.0, nullptr, b1, nb));
+    Epilogue fin;
+    if (sign_only) {
+        fin.s = 1.0; fin.g5 = 1;
+        if (ctx->k > 0) { fin.A1 = low; fin.a1 = 1.0; }
+    } else {
+        fin.s = 1.0 - 0.5 * mass; fin.g5 = 0;
+        fin.A1 = in; fin.a1 = 1.0 + 0.5 * mass;
+        if (ctx->k > 0) { fin.A2 = low; fin.a2 = 1.0 - 0.5 * mass; fin.a_g5 = 2; }
+    }
+    return clenshaw_t<double2>(ctx, ctx->coef.data(), order, x, out, fin, b1, b2, t, nb);
 }
 
 // D_ov(m) in at reduced accuracy (the adaptive CG): polynomial truncated to order n <= ctx->order and,

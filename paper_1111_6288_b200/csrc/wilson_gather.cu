@@ -25,6 +25,8 @@ struct GatherArgs {
     long long V;
     double kappa;
     int reverse;
+    int nrb;               // rhs groups per site block (batched launch): block id = site_block * nrb + rhs_group
+    long long rhs_stride;  // elements between consecutive right-hand sides in in/out/A1..A3
     EpilogueT<C> ep;
 };
 
@@ -60,12 +62,23 @@ __device__ __forceinline__ void hop(C* __restrict__ acc, const GatherArgs<C>& a,
     reconstruct_add<MU, SIGMA>(acc, g, ph);
 }
 
-// NA: number of epilogue operands A1..A_NA (always filled in order); NA = -1: hop only
-template <typename C, int RECON, int NA, bool BL>
-__global__ void __launch_bounds__(GatherShape<C>::threads, GatherShape<C>::min_blocks)
-wilson_gather_kernel(const GatherArgs<C> a) {
+// NA: number of epilogue operands A1..A_NA (always filled in order); NA = -1: hop only.
+// RB: right-hand sides per block (threadIdx.y).  A batched launch puts the rhs groups of one site block on adjacent
+// block ids, so they run at the same time: the links are read from HBM once per site block, from L2 by the other
+// groups, and from L1 by the second rhs of a block.
+template <typename C, int RECON, int NA, bool BL, int RB>
+__global__ void __launch_bounds__(GatherShape<C>::threads * RB, GatherShape<C>::min_blocks / RB)
+wilson_gather_kernel(GatherArgs<C> a) {
     using R = real_t<C>;
-    const unsigned blk = a.reverse ? gridDim.x - 1 - blockIdx.x : blockIdx.x;
+    const unsigned lin = a.reverse ? gridDim.x - 1 - blockIdx.x : blockIdx.x;
+    const unsigned blk = lin / a.nrb;
+    {
+        const long long off = ((long long)(lin % a.nrb) * RB + threadIdx.y) * a.rhs_stride;
+        a.in += off; a.out += off;
+        if (NA >= 1) a.ep.A1 += off;
+        if (NA >= 2) a.ep.A2 += off;
+        if (NA >= 3) a.ep.A3 += off;
+    }
     const long long i = (long long)blk * blockDim.x + threadIdx.x;
     if (i >= a.V) return;
     long long r = i;
@@ -142,9 +155,23 @@ wilson_gather_kernel(const GatherArgs<C> a) {
     }
 }
 
+// nrhs right-hand sides, `stride` elements apart (in, out and every epilogue operand alike)
 template <typename C>
-static int launch_gather_t(ov_ctx* ctx, const C* gauge, const C* in, C* out, const EpilogueT<C>& ep) {
+static int launch_gather_t(ov_ctx* ctx, const C* gauge, const C* in, C* out, const EpilogueT<C>& ep, int nrhs = 1,
+                           long long stride = 0) {
+    if (nrhs > 1 && (nrhs & 1)) {   // odd batch: pairs first, then the last one alone
+        OV_TRY(launch_gather_t<C>(ctx, gauge, in, out, ep, nrhs - 1, stride));
+        EpilogueT<C> e1 = ep;
+        const long long off = (long long)(nrhs - 1) * stride;
+        if (e1.A1) e1.A1 += off;
+        if (e1.A2) e1.A2 += off;
+        if (e1.A3) e1.A3 += off;
+        return launch_gather_t<C>(ctx, gauge, in + off, out + off, e1, 1, 0);
+    }
+    const int rb = nrhs > 1 ? 2 : 1;
     GatherArgs<C> a;
+    a.nrb = nrhs / rb;
+    a.rhs_stride = stride;
     a.gauge = gauge;
     a.in = in;
     a.out = out;
@@ -159,13 +186,18 @@ static int launch_gather_t(ov_ctx* ctx, const C* gauge, const C* in, C* out, con
     ctx->flip ^= 1;
 #endif
     const int threads = GatherShape<C>::threads;
-    const unsigned blocks = (unsigned)((a.V + threads - 1) / threads);
+    const unsigned blocks = (unsigned)((a.V + threads - 1) / threads) * (unsigned)a.nrb;
+    const dim3 bdim(threads, rb);
     const int na = ep.hop_only ? -1 : (ep.A3 ? 3 : ep.A2 ? 2 : ep.A1 ? 1 : 0);
     if ((ep.A3 && !ep.A2) || (ep.A2 && !ep.A1)) return fail(ctx, OV_EINVAL, "epilogue operands must be filled in order");
-#define OV_GATHER(R, N)                                                                                  \
+#define OV_GATHER_B(R, N, B)                                                                             \
     do {                                                                                                 \
-        if (ctx->blocked) wilson_gather_kernel<C, R, N, true><<<blocks, threads, 0, ctx->stream>>>(a);   \
-        else wilson_gather_kernel<C, R, N, false><<<blocks, threads, 0, ctx->stream>>>(a);               \
+        if (ctx->blocked) wilson_gather_kernel<C, R, N, true, B><<<blocks, bdim, 0, ctx->stream>>>(a);   \
+        else wilson_gather_kernel<C, R, N, false, B><<<blocks, bdim, 0, ctx->stream>>>(a);               \
+    } while (0)
+#define OV_GATHER(R, N)                                        \
+    do {                                                       \
+        if (rb == 2) OV_GATHER_B(R, N, 2); else OV_GATHER_B(R, N, 1); \
     } while (0)
 #define OV_GATHER_NA(R)                                 \
     switch (na) {                                       \
@@ -178,6 +210,7 @@ static int launch_gather_t(ov_ctx* ctx, const C* gauge, const C* in, C* out, con
     if (ctx->recon == 12) { OV_GATHER_NA(12) } else { OV_GATHER_NA(18) }
 #undef OV_GATHER_NA
 #undef OV_GATHER
+#undef OV_GATHER_B
     ctx->launches++;
     OV_CUDA(ctx, cudaGetLastError());
     return OV_OK;
@@ -185,6 +218,9 @@ static int launch_gather_t(ov_ctx* ctx, const C* gauge, const C* in, C* out, con
 
 int launch_wilson_gather(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep) {
     return launch_gather_t<double2>(ctx, ctx->gauge, in, out, ep);
+}
+int launch_wilson_batch(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep, int nrhs) {
+    return launch_gather_t<double2>(ctx, ctx->gauge, in, out, ep, nrhs, (long long)spinor_elems(ctx));
 }
 int launch_wilson_gather_f32(ov_ctx* ctx, const float2* in, float2* out, const EpilogueF& ep) {
     if (!ctx->gauge_f) return fail(ctx, OV_ESTATE, "fp32 links have not been made");

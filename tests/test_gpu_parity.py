@@ -284,3 +284,23 @@ def test_adaptive_multishift_cg(ovp, cfg0, mode):
     g0, g1 = to_host(op, x0), to_host(op, x1)
     for i in range(len(masses)):
         assert rel(g1[i], g0[i]) <= 1e-6
+
+
+# ------------------------------------------------------------------------------------------ batched right-hand sides
+@pytest.mark.parametrize("with_small", [True, False])
+def test_batched_apply_matches_single_and_oracle(ovp, cfg0, with_small):
+    """nrhs > 1 goes through batched Wilson launches (2 rhs per block, up to 4 per sweep): same arithmetic per rhs."""
+    c = cfg0
+    cfg = c["cfg"]
+    op, coef = setup_op(ovp, c, with_small=with_small)
+    V, lam = (c["V"], c["lam"]) if with_small else (None, None)
+    xs = np.stack([wl.gaussian_source(cfg.dims, 50 + j) for j in range(7)])   # 4 + 3: a full and a ragged batch
+    d = to_dev(op, xs)
+    got_d, got_s, got_h = to_host(op, op.apply_dov(0.05, d)), to_host(op, op.apply_sign(d)), to_host(op, op.apply_hw(d))
+    for j in range(len(xs)):
+        dj = to_dev(op, xs[j])
+        assert np.array_equal(got_d[j], to_host(op, op.apply_dov(0.05, dj)))
+        assert np.array_equal(got_s[j], to_host(op, op.apply_sign(dj)))
+        assert np.array_equal(got_h[j], to_host(op, op.apply_hw(dj)))
+    ref = oracle.dov(cfg.dims, cfg.kappa, c["U"], coef, cfg.eps, cfg.norm, V, lam, 0.05, xs[6])
+    assert rel(got_d[6], ref) <= TOL_DOV
