@@ -356,6 +356,28 @@ def run_b200(args):
     del a, b
     hw_gbs = (384.0 + 32.0 * args.recon) * V_sites * nhw / (ms_hw * 1e-3) / 1e9
 
+    # ---- the same step with 12-real links (row 3 of every SU(3) link rebuilt in registers): reported beside the headline
+    recon12 = None
+    if args.recon == 18 and not args.no_e2e:
+        op12 = ovp.Overlap(cfg.dims, cfg.kappa, U, recon=12)
+        op12.set_polynomial(coef, cfg.eps, cfg.norm)
+        if k > 0:
+            op12.set_smallspace(Vlow, lam)
+        ne = max(2, min(args.steps, 4))
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for i in range(2):
+            op12.apply_dov(0.0, dev_src[i % nsrc], out)
+        barrier()
+        e0.record(op12.stream)
+        for i in range(ne):
+            op12.apply_dov(0.0, dev_src[i % nsrc], out)
+        e1.record(op12.stream)
+        barrier()
+        ms12 = max_over_ranks(e0.elapsed_time(e1), world, "cuda")
+        recon12 = {"value": aggregate_value(world, ne, ms12), "unit": UNIT, "bytes_per_site_per_launch": 768,
+                   "note": "ov_create(recon=12): 384 B/site of links instead of 576; parity <= 1e-10 (tests)"}
+        op12.close()
+
     # ---- batched right-hand sides (reported separately, G17): 4 sources per Clenshaw sweep
     batched = None
     if not args.no_e2e and nsrc >= 4:
@@ -388,7 +410,7 @@ def run_b200(args):
             dist.destroy_process_group()
         return 0
     return finish(args, cfg, order, k, V_sites, world, ms, value, launches, tim, e2e, hw_gbs, ms_hw / nhw,
-                  sampler, lanczos_s, resid, U, log, cg, batched)
+                  sampler, lanczos_s, resid, U, log, cg, batched, recon12)
 
 
 class _Null:
@@ -417,7 +439,7 @@ def ncu_traffic():
 
 
 def finish(args, cfg, order, k, V_sites, world, ms, value, launches, tim, e2e, hw_gbs, hw_ms, sampler,
-           lanczos_s, resid, U, log, cg=None, batched=None):
+           lanczos_s, resid, U, log, cg=None, batched=None, recon12=None):
     peak, peak_src = measured_peak()
     nsign = args.steps
     wl_launches = tim["wilson_launches"]
@@ -448,7 +470,7 @@ def finish(args, cfg, order, k, V_sites, world, ms, value, launches, tim, e2e, h
         "config": {"workload": workload_name(cfg, order, k), "recon": args.recon, "parallelism": f"replicas x{world}",
                    "l2": "inputs larger than L2 (gauge 510 MB + 17 GB of low modes stream every step)",
                    "low_modes": f"GPU Lanczos, max residual {resid:.1e}, {lanczos_s:.0f} s (untimed setup)" if k else "none"},
-        "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu, "cg_time_to_solution": cg, "batched": batched,
+        "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu, "cg_time_to_solution": cg, "batched": batched, "recon12": recon12,
         "paper_context": "paper: ~30 CPU cores per GPU on unnamed 6 GB GPUs vs Cray XT-5 (PAPER.md:9) - context only",
     }
     print(json.dumps(line), flush=True)

@@ -84,7 +84,9 @@ int ov_unpack_spinor(ov_ctx* ctx, const void* abi_dev, void* canonical_dev, int 
 /* ---- Wilson kernel (row a2) -----------------------------------------------------
  * ov_dslash:   out = sum_mu [ s+ (1-gamma_mu) U_mu(x) in(x+mu) + s- (1+gamma_mu) U_mu(x-mu)^+ in(x-mu) ]
  * ov_apply_hw: out = H_w in = gamma5 (in - kappa * dslash(in))      (NOT divided by the norm)
- * in/out: ABI spinors on the device, nrhs of them.                                                   */
+ * in/out: ABI spinors on the device, nrhs of them.  nrhs > 1 (here and in ov_apply_sign/ov_apply_dov) runs batched
+ * launches: two right-hand sides per thread block, up to four per Clenshaw sweep, sharing the link loads; the result
+ * of every right-hand side is bit-identical to the nrhs = 1 call.                                                 */
 int ov_dslash(ov_ctx* ctx, const void* in, void* out, int nrhs);
 int ov_apply_hw(ov_ctx* ctx, const void* in, void* out, int nrhs);
 
