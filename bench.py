@@ -430,10 +430,17 @@ def measured_peak():
 
 
 def ncu_traffic():
-    """dram bytes per launch of the Wilson kernel from the committed `ncu --set full` capture, if any."""
+    """dram bytes per launch of the Wilson kernel from the committed `ncu --set full` summary, if any."""
     try:
-        with open(os.path.join(ROOT, "profiles", "wilson_traffic.json")) as f:
-            return json.load(f)
+        out = {}
+        with open(os.path.join(ROOT, "profiles", "wilson_traffic.csv")) as f:
+            for line in f.read().splitlines()[1:]:
+                key, val = line.split(",", 1)
+                try:
+                    out[key.strip('"')] = float(val)
+                except ValueError:
+                    out[key.strip('"')] = val.strip('"')
+        return out
     except Exception:
         return None
 
