@@ -432,14 +432,14 @@ def measured_peak():
 def ncu_traffic():
     """dram bytes per launch of the Wilson kernel from the committed `ncu --set full` summary, if any."""
     try:
+        import csv
         out = {}
         with open(os.path.join(ROOT, "profiles", "wilson_traffic.csv")) as f:
-            for line in f.read().splitlines()[1:]:
-                key, val = line.split(",", 1)
+            for row in list(csv.reader(f))[1:]:
                 try:
-                    out[key.strip('"')] = float(val)
+                    out[row[0]] = float(row[1])
                 except ValueError:
-                    out[key.strip('"')] = val.strip('"')
+                    out[row[0]] = row[1]
         return out
     except Exception:
         return None
