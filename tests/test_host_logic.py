@@ -69,3 +69,17 @@ def test_no_cpu_fallback(lib):
     dims = (ctypes.c_int * 4)(4, 4, 4, 4)
     rc = lib.ov_create(ctypes.byref(ctx), dims, ctypes.c_double(0.19), ctypes.c_void_p(8), ctypes.c_int(18), None)
     assert rc == ovp.binding.OV_ECUDA and not ctx.value
+
+
+def test_bench_algorithmic_bytes():
+    """bench.py's roofline numerator: per sign, n Clenshaw orders of 2 launches + the final launch."""
+    import bench
+    V = 1000
+    # n = 1: launch 1 (960) + launch 2 (960 + 2 operands, no b_{j+2} yet) + final (960 + x [+ x_low])
+    assert bench.algorithmic_bytes_per_sign(1, V, False) == (960 + (960 + 384) + (960 + 192)) * V
+    assert bench.algorithmic_bytes_per_sign(1, V, True) == (960 + (960 + 384) + (960 + 384)) * V
+    n = 300
+    per_site = bench.algorithmic_bytes_per_sign(n, 1, True)
+    assert per_site == n * 2496 - 192 + 960 + 384          # SURVEY 8d: 2496 B/site per order
+    assert bench.algorithmic_bytes_per_sign(n, 1, True, recon=12) == per_site - (2 * n + 1) * 192
+    assert bench.aggregate_value(1, 8, 1000.0) == 8.0
