@@ -73,8 +73,9 @@ long long ov_launch_count(const ov_ctx* ctx);
  *                 ms inside the small-space projector, kernel launches in it }  and resets the accumulators. */
 int ov_timing_enable(ov_ctx* ctx, int on);
 int ov_timing_read(ov_ctx* ctx, double* out_host);
-/* selects the dslash kernel: 0 = automatic, 1 = gather (one thread per site, cache-reliant),
- * 2 = tiled (shared-memory staged).  Returns OV_EINVAL if the variant cannot run on this lattice. */
+/* selects the dslash kernel: 0 = automatic, 1 = gather (one thread per site, operands through L1/L2).  2 is reserved
+ * for a shared-memory staged kernel; the staged designs measured so far were slower than the gather kernel (DESIGN.md
+ * section 10), none ships, and the call returns OV_EINVAL. */
 int ov_set_dslash_variant(ov_ctx* ctx, int variant);
 
 /* ---- layout ------------------------------------------------------------------- */

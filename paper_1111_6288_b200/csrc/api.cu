@@ -58,8 +58,6 @@ int ensure_reduction_buffers(ov_ctx* ctx, size_t partial_elems, size_t result_el
 }
 
 int launch_wilson(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep) {
-    const int v = ctx->dslash_variant;
-    if (v == 2 || (v == 0 && tiled_supported(ctx))) return launch_wilson_tiled(ctx, in, out, ep);
     return launch_wilson_gather(ctx, in, out, ep);
 }
 
@@ -187,7 +185,7 @@ int ov_timing_read(ov_ctx* ctx, double* out_host) {
 int ov_set_dslash_variant(ov_ctx* ctx, int variant) {
     if (!ctx) return OV_EINVAL;
     if (variant < 0 || variant > 2) return fail(ctx, OV_EINVAL, "variant must be 0, 1 or 2");
-    if (variant == 2 && !tiled_supported(ctx)) return fail(ctx, OV_EINVAL, "tiled dslash does not support this lattice");
+    if (variant == 2) return fail(ctx, OV_EINVAL, "no shared-memory staged Wilson kernel in this build (DESIGN.md section 10)");
     ctx->dslash_variant = variant;
     return OV_OK;
 }

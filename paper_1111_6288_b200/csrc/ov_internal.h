@@ -139,8 +139,6 @@ int launch_wilson_gather(ov_ctx* ctx, const double2* in, double2* out, const Epi
 // batched: nrhs consecutive ABI spinors (stride 12 V) in in/out and in every epilogue operand
 int launch_wilson_batch(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep, int nrhs);
 int launch_wilson_gather_f32(ov_ctx* ctx, const float2* in, float2* out, const EpilogueF& ep);  // needs ctx->gauge_f
-int launch_wilson_tiled(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep);
-bool tiled_supported(const ov_ctx* ctx);
 // host-side dense Hermitian eigensolver (cyclic complex Jacobi): A (n x n, row-major complex, destroyed),
 // w ascending, Z row-major with eigenvectors as COLUMNS
 void host_eigh(int n, std::vector<double2>& A, std::vector<double>& w, std::vector<double2>& Z);

@@ -1,6 +1,5 @@
 // Wilson kernel, variant 1 ("gather"): one thread per lattice site, neighbours read straight from
-// global memory through L1/L2.  Works for every lattice shape; it is
-// the general-shape path and the baseline the tiled kernel (wilson_tiled.cu) is measured against.
+// global memory through L1/L2.  Works for every lattice shape.
 //
 //   out = s * G (in - kappa * hop(in)) + a1*A1 + a2*A2 + a3*A3        (Epilogue, ov_internal.h)
 //   hop(in)(x) = sum_mu [ s+ (1-gamma_mu) U_mu(x) in(x+mu) + s- (1+gamma_mu) U_mu(x-mu)^+ in(x-mu) ]

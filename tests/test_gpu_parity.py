@@ -304,3 +304,22 @@ def test_batched_apply_matches_single_and_oracle(ovp, cfg0, with_small):
         assert np.array_equal(got_h[j], to_host(op, op.apply_hw(dj)))
     ref = oracle.dov(cfg.dims, cfg.kappa, c["U"], coef, cfg.eps, cfg.norm, V, lam, 0.05, xs[6])
     assert rel(got_d[6], ref) <= TOL_DOV
+
+
+def test_timing_hooks_and_launch_count(ovp, cfg0):
+    """bench.py's roofline reads these: every launch inside the Clenshaw sweep is the Wilson kernel (2n+1 per sign)."""
+    op, _ = setup_op(ovp, cfg0)
+    dx = to_dev(op, cfg0["x"])
+    out = torch.empty_like(dx)
+    op.timing_enable(True)
+    l0 = op.launch_count
+    for _ in range(3):
+        op.apply_dov(0.0, dx, out)
+    t = op.timing_read()
+    op.timing_enable(False)
+    n = cfg0["cfg"].order
+    assert t["wilson_launches"] == 3 * (2 * n + 1) and t["wilson_ms"] > 0
+    assert t["projector_launches"] == 3 * 4 and t["projector_ms"] > 0
+    assert op.launch_count - l0 == 3 * (2 * n + 1 + 4 + 1)      # + projector (4) + the b_n = c_n x axpby
+    with pytest.raises(ovp.OvError):
+        op.set_dslash_variant(2)
