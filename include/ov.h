@@ -55,7 +55,9 @@ typedef struct ov_ctx ov_ctx;
  * ov_create: builds a context for one gauge field.  gauge_dev: canonical gauge on the DEVICE; it is
  * COPIED and re-laid out (site-major SoA, row-major 3x3 per link; recon = 18 keeps all 9 complex
  * entries, recon = 12 keeps rows 0-1 and rebuilds row 2 = conj(row0 x row1) in registers, valid for
- * SU(3) links only).  The caller may free gauge_dev after the call returns (the call synchronises).
+ * SU(3) links only: ov_create checks every link and returns OV_EINVAL if one is further than 1e-9 from SU(3); recon = 18
+ * takes ANY complex 3x3 links, e.g. U(3) links carrying a U(1) background-field phase, or zero links
+ * across a Dirichlet boundary).  The caller may free gauge_dev after the call returns (it synchronises).
  * kappa = 1/(2(m0+4)) is the Wilson hopping parameter (reading G1).
  * cuda_stream: a cudaStream_t (NULL = legacy default stream).                                        */
 int ov_create(ov_ctx** out, const int dims[4], double kappa, const void* gauge_dev, int recon,

@@ -123,7 +123,13 @@ int ov_create(ov_ctx** out, const int dims[4], double kappa, const void* gauge_d
     const size_t gbytes = gauge_elems(ctx->lat.V, recon) * sizeof(double2);
     cudaError_t e = cudaMalloc(&ctx->gauge, gbytes);
     if (e != cudaSuccess) { delete ctx; return e == cudaErrorMemoryAllocation ? OV_ENOMEM : OV_ECUDA; }
-    int rc = launch_gauge_relayout(ctx, (const double2*)gauge_dev);
+    int rc = OV_OK;
+    if (recon == 12) {   // rows 0-1 only make sense if row 2 really is conj(row0 x row1)
+        double defect = 0.0;
+        rc = gauge_su3_defect(ctx, (const double2*)gauge_dev, &defect);
+        if (rc == OV_OK && !(defect <= 1e-9)) rc = OV_EINVAL;
+    }
+    if (rc == OV_OK) rc = launch_gauge_relayout(ctx, (const double2*)gauge_dev);
     if (rc == OV_OK && cudaStreamSynchronize(ctx->stream) != cudaSuccess) rc = OV_ECUDA;
     if (rc == OV_OK) rc = ensure_reduction_buffers(ctx, 1, 1024);
     if (rc != OV_OK) { ov_destroy(ctx); return rc; }

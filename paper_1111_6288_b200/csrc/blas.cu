@@ -4,6 +4,7 @@
 // Reductions are two-stage with a fixed shape (warp shuffle -> per-warp partial in global memory ->
 // one block per result summing the partials in a fixed tree), no atomics: bit-reproducible.
 #include <algorithm>
+#include <cstring>
 
 #include "ov_internal.h"
 #include "wilson_math.cuh"
@@ -20,6 +21,48 @@ __global__ void gauge_relayout_kernel(const double2* __restrict__ can, double2* 
     for (int mu = 0; mu < 4; mu++)
 #pragma unroll
         for (int e = 0; e < NE; e++) g[gauge_index<NE, BL>(V, mu, e, i)] = can[(i * 4 + mu) * 9 + e];
+}
+
+// largest |row2 - conj(row0 x row1)| and |<row_i,row_j> - delta_ij| over all links: recon 12 is only valid for SU(3)
+__global__ void su3_defect_kernel(const double2* __restrict__ can, long long nlinks, unsigned long long* worst) {
+    const long long l = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (l >= nlinks) return;
+    double2 u[9], r[9];
+#pragma unroll
+    for (int e = 0; e < 9; e++) { u[e] = can[l * 9 + e]; r[e] = u[e]; }
+    su3_row2(r);
+    double d = 0.0;
+#pragma unroll
+    for (int e = 6; e < 9; e++) d = fmax(d, fmax(fabs(r[e].x - u[e].x), fabs(r[e].y - u[e].y)));
+#pragma unroll
+    for (int i = 0; i < 2; i++)
+#pragma unroll
+        for (int j = i; j < 2; j++) {
+            double2 acc = make_double2(0.0, 0.0);
+#pragma unroll
+            for (int c = 0; c < 3; c++) cmaddc(acc, u[3 * i + c], u[3 * j + c]);
+            d = fmax(d, fmax(fabs(acc.x - (i == j ? 1.0 : 0.0)), fabs(acc.y)));
+        }
+    atomicMax(worst, (unsigned long long)__double_as_longlong(d));   // non-negative doubles order like integers
+}
+
+int gauge_su3_defect(ov_ctx* ctx, const double2* canonical, double* defect) {
+    unsigned long long* d_w = nullptr;
+    OV_CUDA(ctx, cudaMalloc(&d_w, sizeof(unsigned long long)));
+    OV_CUDA(ctx, cudaMemsetAsync(d_w, 0, sizeof(unsigned long long), ctx->stream));
+    const long long nlinks = 4 * ctx->lat.V;
+    su3_defect_kernel<<<(unsigned)((nlinks + 127) / 128), 128, 0, ctx->stream>>>(canonical, nlinks, d_w);
+    ctx->launches++;
+    unsigned long long h = 0;
+    cudaError_t e = cudaMemcpyAsync(&h, d_w, sizeof h, cudaMemcpyDeviceToHost, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    cudaFree(d_w);
+    OV_CUDA(ctx, e);
+    long long bits = (long long)h;
+    double v;
+    memcpy(&v, &bits, sizeof v);
+    *defect = v;
+    return OV_OK;
 }
 
 int launch_gauge_relayout(ov_ctx* ctx, const double2* canonical) {

@@ -132,6 +132,7 @@ int ensure_reduction_buffers(ov_ctx* ctx, size_t partial_elems, size_t result_el
 
 // --- kernels (launchers); all enqueue on ctx->stream and bump ctx->launches ---
 int launch_gauge_relayout(ov_ctx* ctx, const double2* canonical);
+int gauge_su3_defect(ov_ctx* ctx, const double2* canonical, double* defect);
 int launch_pack(ov_ctx* ctx, const double2* canonical, double2* abi);
 int launch_unpack(ov_ctx* ctx, const double2* abi, double2* canonical);
 int launch_wilson(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep);

@@ -323,3 +323,22 @@ def test_timing_hooks_and_launch_count(ovp, cfg0):
     assert op.launch_count - l0 == 3 * (2 * n + 1 + 4 + 1)      # + projector (4) + the b_n = c_n x axpby
     with pytest.raises(ovp.OvError):
         op.set_dslash_variant(2)
+
+
+# ------------------------------------------------------------------------------------------ links that are not SU(3)
+def test_u3_and_dirichlet_links(ovp):
+    """recon 18 takes any 3x3 links: a U(1) background phase on every link (U -> e^{-iqA} U) and zero links
+    across a Dirichlet boundary in x and t; recon 12 must refuse them (row 2 could not be rebuilt)."""
+    dims = (4, 2, 6, 8)
+    U = wl.su3_links(dims, 0.6, 31)
+    rng = np.random.default_rng(32)
+    phase = np.exp(-1j * 0.7 * rng.standard_normal(U.shape[:5]))          # one U(1) phase per link
+    Ub = U * phase[..., None, None]
+    Ub[:, :, :, -1, 0] = 0.0                                               # no hop across the x boundary
+    Ub[-1, :, :, :, 3] = 0.0                                               # nor across the t boundary
+    x = wl.gaussian_source(dims, 33)
+    op = make(ovp, dims, Ub, recon=18)
+    assert rel(to_host(op, op.apply_hw(to_dev(op, x))), oracle.hw(dims, KAPPA, Ub, x)) <= TOL_HW
+    with pytest.raises(ovp.OvError):
+        make(ovp, dims, Ub, recon=12)
+    make(ovp, dims, U, recon=12)                                           # genuine SU(3) links are accepted
