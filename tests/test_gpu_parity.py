@@ -342,3 +342,31 @@ def test_u3_and_dirichlet_links(ovp):
     with pytest.raises(ovp.OvError):
         make(ovp, dims, Ub, recon=12)
     make(ovp, dims, U, recon=12)                                           # genuine SU(3) links are accepted
+
+
+# ------------------------------------------------------------------------------------------ degenerate cases
+def test_degenerate_inputs(ovp, cfg0):
+    c = cfg0
+    cfg = c["cfg"]
+    op, _ = setup_op(ovp, c)
+    zero = torch.zeros_like(to_dev(op, c["x"]))
+    # zero source: nothing to solve
+    x, iters, res, ok = op.multishift_cg((0.1, 0.02), zero, tol=1e-8, maxiter=50)
+    assert ok and iters == 0 and float(x.abs().max()) == 0.0 and np.all(res == 0.0)
+    # iteration limit reached: flagged, the last iterate is returned, true residuals are still reported
+    x, iters, res, ok = op.multishift_cg((0.1, 0.02), to_dev(op, c["x"]), tol=1e-12, maxiter=2)
+    assert not ok and iters == 2 and np.all(np.isfinite(res)) and np.all(res > 1e-12)
+    # operators are linear: the zero vector maps to the zero vector, in every entry point
+    for y in (op.apply_hw(zero), op.apply_sign(zero), op.apply_dov(0.3, zero), op.dslash(zero)):
+        assert float(y.abs().max()) == 0.0
+    # bad arguments
+    with pytest.raises(ovp.OvError):
+        op.lanczos_lowmodes(0)
+    with pytest.raises(ovp.OvError):
+        op.lanczos_lowmodes(4, subspace=12 * op.V)           # Krylov space as large as the whole space
+    with pytest.raises(ovp.OvError):
+        op.multishift_cg((2.5,), zero)                       # mass outside (-2, 2)
+    with pytest.raises(ovp.OvError):
+        op.apply_dov_reduced(0.0, zero, cfg.order + 1, False)
+    with pytest.raises(ovp.OvError):
+        ovp.Overlap((4, 4, 4, 1), KAPPA, wl.unit_links((4, 4, 4, 1)))   # every extent must be >= 2
