@@ -50,6 +50,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cg", action="store_true")
+    ap.add_argument("--kernels", action="store_true",
+                    help="time every kernel class of the path alone (CUDA events) and print a per-kernel roofline table")
     return ap.parse_args()
 
 
@@ -484,10 +486,78 @@ def finish(args, cfg, order, k, V_sites, world, ms, value, launches, tim, e2e, h
     return 0
 
 
+def run_kernels(args):
+    """Per-kernel table: each entry point that is one kernel class, timed alone with CUDA events on the library's stream,
+    algorithmic bytes as in DESIGN.md section 6 (operands of 170 MB each, so nothing lives in L2 between launches)."""
+    import torch
+    import paper_1111_6288_b200 as ovp
+    from paper_1111_6288_b200 import build as ovbuild
+    ovbuild.build()
+    torch.cuda.set_device(0)
+    cfg = wl.CONFIGS[args.config]
+    V = wl.volume(cfg.dims)
+    U = wl.su3_links(cfg.dims, cfg.spread, wl.gauge_seed(cfg.index))
+    op = ovp.Overlap(cfg.dims, cfg.kappa, U, recon=18)
+    op12 = ovp.Overlap(cfg.dims, cfg.kappa, U, recon=12)
+    peak, peak_src = measured_peak()
+    k = 16  # a small stand-in basis is enough to time the projector kernels per vector
+    xs = [op.pack_spinor(torch.from_numpy(wl.gaussian_source(cfg.dims, 100 + j)).cuda()) for j in range(2)]
+    x, y = xs
+    Vb = torch.stack([x, y] * (k // 2)).contiguous()
+    Vb = Vb / torch.linalg.norm(Vb.reshape(k, -1), dim=1).reshape(k, 1, 1)
+    op.set_polynomial(ovp.chebyshev_coeffs(8, cfg.eps), cfg.eps, cfg.norm)
+    op.set_smallspace(Vb, np.where(np.arange(k) % 2 == 0, 0.05, -0.05))
+    x4, y4 = torch.stack([x, y, x, y]).contiguous(), torch.empty(4, *x.shape, dtype=x.dtype, device=x.device)
+    can = op.unpack_spinor(x)
+    S = 192.0 * V  # bytes of one spinor
+
+    def t(fn, reps):
+        for _ in range(3):
+            fn()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(op.stream)
+        for _ in range(reps):
+            fn()
+        e1.record(op.stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    table = {}
+
+    def add(name, nbytes, fn, reps=50):
+        ms = t(fn, reps)
+        table[name] = {"ms": ms, "algorithmic_MB": nbytes / 1e6, "GB/s": nbytes / (ms * 1e-3) / 1e9,
+                       "frac_of_measured_hbm": nbytes / (ms * 1e-3) / 1e9 / peak}
+
+    out = torch.empty_like(x)
+    torch.cuda.cudart().cudaProfilerStart()
+    add("wilson_gather<18> H_w (ov_apply_hw)", 960.0 * V, lambda: op.apply_hw(x, out))
+    add("wilson_gather<18> hop only (ov_dslash)", 960.0 * V, lambda: op.dslash(x, out))
+    add("wilson_gather<12> H_w (recon 12)", 768.0 * V, lambda: op12.apply_hw(x, out))
+    add("wilson_gather<18> batched, 4 rhs per launch", (4 * 384.0 + 576.0) * V, lambda: op.apply_hw(x4, y4), 20)
+    add("axpy (ov_blas_axpy)", 3 * S, lambda: op.blas_axpy(0.5 + 0.25j, x, out))
+    add("scale (ov_blas_scale)", 2 * S, lambda: op.blas_scale(1.0, out))
+    add("dot1 + reduce_partials (ov_blas_dot, incl. the host synchronisation)", 2 * S, lambda: op.blas_dot(x, y))
+    add("pack (ov_pack_spinor)", 2 * S, lambda: op.pack_spinor(can))
+    add("unpack (ov_unpack_spinor)", 2 * S, lambda: op.unpack_spinor(x))
+    add(f"projector k={k}: multi_dot + coef + multi_axpy<2> (ov_project, incl. host copy of c)", (2 * k + 4) * S,
+        lambda: op.project(x), 20)
+    add("D_ov reduced, order 8, fp64 sweep (17 Wilson launches + projector)", 0.0, lambda: op.apply_dov_reduced(0.0, x, 8, False, out), 10)
+    add("D_ov reduced, order 8, fp32 sweep (17 fp32 Wilson launches + projector + conversions)", 0.0,
+        lambda: op.apply_dov_reduced(0.0, x, 8, True, out), 10)
+    torch.cuda.cudart().cudaProfilerStop()
+    print(json.dumps({"impl": "kernels", "config": {"workload": f"configs[{cfg.index}] {cfg.name}", "sites": V},
+                      "peak_GB/s": peak, "peak_source": peak_src, "kernels": table}), flush=True)
+    return 0
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.kernels:
+        return run_kernels(args)
     return run_b200(args)
 
 

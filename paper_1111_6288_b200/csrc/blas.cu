@@ -344,8 +344,40 @@ int fetch_results(ov_ctx* ctx, int n, double2* host_out) {
     return OV_OK;
 }
 
+// one plain dot product <x, y>: 8 independent 16-byte loads per thread and pass, fixed-shape reduction
+constexpr int kDot1Threads = 256;
+constexpr int kDot1E = 4;
+__global__ void __launch_bounds__(kDot1Threads) dot1_kernel(const double2* __restrict__ x, const double2* __restrict__ y,
+                                                            long long n, double2* __restrict__ partial) {
+    __shared__ double2 sh[kDot1Threads];
+    const long long base = (long long)blockIdx.x * (kDot1Threads * kDot1E) + threadIdx.x;
+    double2 xv[kDot1E], yv[kDot1E];
+#pragma unroll
+    for (int m = 0; m < kDot1E; m++) {
+        const long long e = base + (long long)m * kDot1Threads;
+        xv[m] = (e < n) ? x[e] : make_double2(0.0, 0.0);
+        yv[m] = (e < n) ? y[e] : make_double2(0.0, 0.0);
+    }
+    double2 acc = make_double2(0.0, 0.0);
+#pragma unroll
+    for (int m = 0; m < kDot1E; m++) cmaddc(acc, xv[m], yv[m]);
+    sh[threadIdx.x] = acc;
+    __syncthreads();
+    for (int o = kDot1Threads / 2; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) sh[threadIdx.x] = cadd(sh[threadIdx.x], sh[threadIdx.x + o]);
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) partial[blockIdx.x] = sh[0];
+}
+
 int dot_host(ov_ctx* ctx, const double2* x, const double2* y, double2* out) {
-    OV_TRY(launch_multi_dot(ctx, x, 0, 1, y));
+    const long long n = (long long)spinor_elems(ctx);
+    const long long nblocks = (n + kDot1Threads * kDot1E - 1) / (kDot1Threads * kDot1E);
+    OV_TRY(ensure_reduction_buffers(ctx, (size_t)nblocks, 1));
+    dot1_kernel<<<(unsigned)nblocks, kDot1Threads, 0, ctx->stream>>>(x, y, n, ctx->d_partial);
+    reduce_partials_kernel<<<1, kRedThreads, 0, ctx->stream>>>(ctx->d_partial, nblocks, ctx->d_result);
+    ctx->launches += 2;
+    OV_CUDA(ctx, cudaGetLastError());
     return fetch_results(ctx, 1, out);
 }
 int norm2_host(ov_ctx* ctx, const double2* x, double* out) {
