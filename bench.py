@@ -52,6 +52,7 @@ def parse_args():
     ap.add_argument("--no-cg", action="store_true")
     ap.add_argument("--kernels", action="store_true",
                     help="time every kernel class of the path alone (CUDA events) and print a per-kernel roofline table")
+    ap.add_argument("--reps", type=int, default=0, help="with --kernels: launches per kernel class (0 = defaults)")
     return ap.parse_args()
 
 
@@ -526,7 +527,7 @@ def run_kernels(args):
     table = {}
 
     def add(name, nbytes, fn, reps=50):
-        ms = t(fn, reps)
+        ms = t(fn, args.reps if args.reps > 0 else reps)
         table[name] = {"ms": ms, "algorithmic_MB": nbytes / 1e6, "GB/s": nbytes / (ms * 1e-3) / 1e9,
                        "frac_of_measured_hbm": nbytes / (ms * 1e-3) / 1e9 / peak}
 
