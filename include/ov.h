@@ -147,7 +147,7 @@ int ov_blas_norm2(ov_ctx* ctx, const void* x, double* out_host);
  *   subspace = Krylov dimension m (0 = default: 2k+16, reduced to what fits in free device memory; the paper uses
  *   2.5 k); cheb_order = degree of the filter in Q^2 (paper: 100).
  *   Memory: V_out_dev itself holds the first k basis vectors during the call (its contents are scratch until the
- *   call returns); the library allocates the other m+1-k basis vectors + 3 spinors and frees them before returning.
+ *   call returns); the library allocates the other m+1-k basis vectors + 2 spinors and frees them before returning.
  *   All basis rotations are done in place, so k = 200 on 32^3x64 (80.5 GB of V) fits in 180 GB.                    */
 /* ov_set_cg_adaptive ("adaptive CG": lower polynomial order as the CG converges, then single precision):
  *   mode 0 (default): every operator application at full order in fp64;

@@ -39,7 +39,7 @@ struct Filter {
 // out = T_d(z(Q^2)) in ; t1, tq: scratch spinors distinct from in/out.  T_j lives in `out` when j has the parity
 // of d and in t1 otherwise; from j = 3 on each T_j is written in place over T_{j-2} (the epilogue reads its
 // axpy operands at the output site only).
-static int apply_filter(ov_ctx* ctx, const Filter& f, const double2* in, double2* out, double2* /*t0*/, double2* t1,
+static int apply_filter(ov_ctx* ctx, const Filter& f, const double2* in, double2* out, double2* t1,
                         double2* tq) {
     const double inv = 1.0 / ctx->norm, w = f.b - f.a, cs = (f.a + f.b) / w;
     auto buf = [&](int j) { return ((j & 1) == (f.d & 1)) ? out : t1; };
@@ -132,7 +132,7 @@ extern "C" int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_resta
     if (m < m_min) m = m_min;
     if ((long long)m >= dim) return fail(ctx, OV_EINVAL, "subspace %d too large for dimension %lld", m, dim);
     if ((size_t)m * kRotTileBytesPerVector > 220 * 1024) m = (int)(220 * 1024 / kRotTileBytesPerVector);
-    {   // fit the pool into free memory: vectors k..m of the basis + 3 scratch (+ 2 GB head room for the workspaces)
+    {   // fit the pool into free memory: vectors k..m of the basis + 2 scratch (+ 2 GB head room for the workspaces)
         size_t free_b = 0, total_b = 0;
         OV_CUDA(ctx, cudaMemGetInfo(&free_b, &total_b));
         const size_t head = (size_t)2 << 30;
@@ -141,8 +141,8 @@ extern "C" int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_resta
         if (m < m_min) return fail(ctx, OV_ENOMEM, "lanczos: %d basis vectors do not fit in free device memory", m_min + 1);
     }
 
-    double2* pool = nullptr;  // basis vectors k..m, then 3 scratch
-    const size_t npool = (size_t)(m + 1 - k) + 3;
+    double2* pool = nullptr;  // basis vectors k..m, then 2 scratch
+    const size_t npool = (size_t)(m + 1 - k) + 2;
     OV_CUDA(ctx, cudaMalloc(&pool, bytes * npool));
     double2 *d_C = nullptr, *d_St = nullptr;
     if (cudaMalloc(&d_C, (size_t)(m + 1) * sizeof(double2)) != cudaSuccess ||
@@ -154,7 +154,6 @@ extern "C" int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_resta
     const Basis W{(double2*)V_out_dev, k, pool, n};
     double2* t1 = pool + (size_t)(m + 1 - k) * n;
     double2* tq = t1 + n;
-    double2* t0 = tq + n;
 
     auto normalise = [&](double2* v, double* nrm) -> int {
         double s;
@@ -203,7 +202,7 @@ extern "C" int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_resta
     for (int restart = 0; restart < max_restarts; restart++) {
         for (int j = l; j < m; j++) {
             double2* u = W.vec(j + 1);
-            OV_TRY(apply_filter(ctx, f, W.vec(j), u, t0, t1, tq));
+            OV_TRY(apply_filter(ctx, f, W.vec(j), u, t1, tq));
             OV_TRY(cgs_pass(ctx, W, j + 1, u, d_C, c));
             double alpha = c[j].x;
             OV_TRY(cgs_pass(ctx, W, j + 1, u, d_C, c));
