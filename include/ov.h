@@ -79,6 +79,8 @@ int ov_timing_read(ov_ctx* ctx, double* out_host);
  * for a shared-memory staged kernel; the staged designs measured so far were slower than the gather kernel (DESIGN.md
  * section 10), none ships, and the call returns OV_EINVAL. */
 int ov_set_dslash_variant(ov_ctx* ctx, int variant);
+/* the variant single-right-hand-side Wilson launches of this context actually use (1 or 2; never 0) */
+int ov_get_dslash_variant(const ov_ctx* ctx);
 
 /* ---- layout ------------------------------------------------------------------- */
 int ov_pack_spinor(ov_ctx* ctx, const void* canonical_dev, void* abi_dev, int nrhs);
@@ -123,6 +125,9 @@ int ov_apply_dov(ov_ctx* ctx, double mass, const void* in, void* out, int nrhs);
  * caller's Chebyshev series truncated to `order` <= the order set, and with use_f32 != 0 the Clenshaw sweep runs in
  * single precision (links and Clenshaw vectors in fp32; projector, in, out and the D_ov assembly stay fp64).  One RHS. */
 int ov_apply_dov_reduced(ov_ctx* ctx, double mass, const void* in, void* out, int order, int use_f32);
+/* test/bench hook: out = H_w in computed by the SINGLE-precision instantiation of the Wilson kernel (in is rounded to
+ * fp32, the links are the fp32 copy the adaptive CG uses, the result is widened to fp64).  One right-hand side.       */
+int ov_apply_hw_f32(ov_ctx* ctx, const void* in, void* out);
 int ov_apply_hw_host(ov_ctx* ctx, const void* in_host, void* out_host, int nrhs);
 int ov_apply_dov_host(ov_ctx* ctx, double mass, const void* in_host, void* out_host, int nrhs);
 
@@ -153,7 +158,9 @@ int ov_blas_norm2(ov_ctx* ctx, const void* x, double* out_host);
  *   mode 0 (default): every operator application at full order in fp64;
  *   mode 1: at iteration j the application of A only needs relative accuracy eta_j ~ tol |b| / |r_j| (inexact-Krylov
  *           relaxation), so the series is truncated to the smallest order whose difference from the full polynomial,
- *           measured on [min(eps, lambda_k^2), 1], is below eta_j;
+ *           measured on [max(eps, 0.96 max_i lambda_i^2), 1], is below eta_j.  PRECONDITION: the small space set by
+ *           ov_set_smallspace is complete below max|lambda_i| (holds every mode of Q with |lambda| < max|lambda_i|, as
+ *           ov_lanczos_lowmodes returns); with an incomplete set the reduced sweeps are inaccurate on the missing modes;
  *   mode 2: mode 1, and the Clenshaw sweep runs in fp32 once eta_j is above the fp32 rounding floor.
  * The CG vectors and recurrences stay fp64; the true residuals reported at the end always use the full operator. */
 int ov_set_cg_adaptive(ov_ctx* ctx, int mode);
@@ -163,6 +170,10 @@ int ov_multishift_cg(ov_ctx* ctx, const double* masses_host, int nmass, const vo
                      int maxiter, int* iters_out, double* relres_out);
 int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_restarts, int cheb_order, int subspace,
                         void* V_out_dev, double* lambda_out_host, double* resid_out_host);
+/* statistics of the last ov_lanczos_lowmodes call: out_host[6] = { restart cycles, filter applications (each 2*cheb_order
+ * Wilson launches), kernel launches in the call, final lower edge a of the filter window [a,1] of Q^2 (modes with
+ * lambda^2 < a are amplified), times the window had to be widened (completeness guard), Krylov dimension m }.  */
+int ov_lanczos_stats(const ov_ctx* ctx, double* out_host);
 
 /* ---- host-logic test hook (no device work): eigen-decomposition of a dense n x n Hermitian matrix by the
  * cyclic complex Jacobi routine the Lanczos driver uses.  A_host: row-major (re,im) pairs; w_out: n ascending

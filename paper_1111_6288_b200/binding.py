@@ -22,10 +22,10 @@ _CODES = {1: "OV_EINVAL", 2: "OV_ENOMEM", 3: "OV_ECUDA", 4: "OV_ESTATE", 5: "OV_
 SYMBOLS = [
     "ov_create", "ov_destroy", "ov_last_error", "ov_spinor_bytes", "ov_volume", "ov_spinor_layout", "ov_launch_count",
     "ov_timing_enable", "ov_timing_read",
-    "ov_set_dslash_variant", "ov_pack_spinor", "ov_unpack_spinor", "ov_dslash", "ov_apply_hw",
+    "ov_set_dslash_variant", "ov_get_dslash_variant", "ov_pack_spinor", "ov_unpack_spinor", "ov_dslash", "ov_apply_hw",
     "ov_chebyshev_coeffs", "ov_set_polynomial", "ov_set_smallspace", "ov_project", "ov_apply_sign",
-    "ov_apply_dov", "ov_apply_dov_reduced", "ov_set_cg_adaptive", "ov_cg_orders", "ov_apply_hw_host", "ov_apply_dov_host", "ov_blas_axpy", "ov_blas_scale", "ov_blas_dot",
-    "ov_blas_norm2", "ov_multishift_cg", "ov_lanczos_lowmodes", "ov_host_eigh",
+    "ov_apply_dov", "ov_apply_dov_reduced", "ov_apply_hw_f32", "ov_set_cg_adaptive", "ov_cg_orders", "ov_apply_hw_host", "ov_apply_dov_host", "ov_blas_axpy", "ov_blas_scale", "ov_blas_dot",
+    "ov_blas_norm2", "ov_multishift_cg", "ov_lanczos_lowmodes", "ov_lanczos_stats", "ov_host_eigh",
 ]
 
 
@@ -156,6 +156,10 @@ class Overlap:
         self._check(self.lib.ov_timing_read(self._ctx, out))
         return dict(wilson_ms=out[0], wilson_launches=int(out[1]), projector_ms=out[2], projector_launches=int(out[3]))
 
+    @property
+    def dslash_variant(self):
+        return int(self.lib.ov_get_dslash_variant(self._ctx))
+
     def set_dslash_variant(self, v):
         self._check(self.lib.ov_set_dslash_variant(self._ctx, ctypes.c_int(v)))
 
@@ -198,6 +202,11 @@ class Overlap:
         out = torch.empty_like(x) if out is None else out
         self._check(self.lib.ov_apply_dov_reduced(self._ctx, ctypes.c_double(mass), _ptr(x), _ptr(out), ctypes.c_int(order),
                                                   ctypes.c_int(1 if use_f32 else 0)))
+        return out
+
+    def apply_hw_f32(self, x, out=None):
+        out = torch.empty_like(x) if out is None else out
+        self._check(self.lib.ov_apply_hw_f32(self._ctx, _ptr(x), _ptr(out)))
         return out
 
     def set_cg_adaptive(self, mode):
@@ -291,3 +300,10 @@ class Overlap:
         if rc not in (OV_OK, OV_ENOCONV):
             self._check(rc)
         return V, lam, res, rc == OV_OK
+
+    def lanczos_stats(self):
+        """ov_lanczos_stats: counters of the last lanczos_lowmodes call."""
+        out = (ctypes.c_double * 6)()
+        self._check(self.lib.ov_lanczos_stats(self._ctx, out))
+        return dict(restarts=int(out[0]), filter_applies=int(out[1]), launches=int(out[2]), edge=out[3],
+                    widenings=int(out[4]), subspace=int(out[5]))

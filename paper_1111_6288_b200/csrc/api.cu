@@ -57,6 +57,8 @@ int ensure_reduction_buffers(ov_ctx* ctx, size_t partial_elems, size_t result_el
     return OV_OK;
 }
 
+int effective_variant(const ov_ctx* ctx) { return 1; }
+
 int launch_wilson(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep) {
     return launch_wilson_gather(ctx, in, out, ep);
 }
@@ -109,6 +111,7 @@ int ov_create(ov_ctx** out, const int dims[4], double kappa, const void* gauge_d
     if (recon != 18 && recon != 12) return OV_EINVAL;
     for (int d = 0; d < 4; d++)
         if (dims[d] < 2) return OV_EINVAL;
+    if (!(kappa > 0.0) || !std::isfinite(kappa)) return OV_EINVAL;  // the kernel forms in/kappa (own term first)
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return OV_ECUDA;  // no CPU fallback
     ov_ctx* ctx = new ov_ctx();
@@ -195,6 +198,8 @@ int ov_set_dslash_variant(ov_ctx* ctx, int variant) {
     ctx->dslash_variant = variant;
     return OV_OK;
 }
+
+int ov_get_dslash_variant(const ov_ctx* ctx) { return ctx ? effective_variant(ctx) : 0; }
 
 int ov_pack_spinor(ov_ctx* ctx, const void* canonical_dev, void* abi_dev, int nrhs) {
     OV_TRY(check_apply(ctx, canonical_dev, abi_dev, nrhs));

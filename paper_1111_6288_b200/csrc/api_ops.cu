@@ -128,6 +128,20 @@ int ov_apply_dov_reduced(ov_ctx* ctx, double mass, const void* in, void* out, in
     return apply_dov_reduced(ctx, mass, (const double2*)in, (double2*)out, order, use_f32 != 0);
 }
 
+// test/bench hook for the fp32 instantiation of the Wilson kernel (the adaptive CG's single-precision sweeps):
+// in -> fp32, H_w with the fp32 copy of the links, result widened back to fp64.
+int ov_apply_hw_f32(ov_ctx* ctx, const void* in, void* out) {
+    OV_TRY(check2(ctx, in, out, 1));
+    OV_TRY(ensure_gauge_f32(ctx));
+    float2 *xf, *yf;
+    OV_TRY(workspace_f32(ctx, 0, &xf));
+    OV_TRY(workspace_f32(ctx, 1, &yf));
+    OV_TRY(launch_scale_to_f32(ctx, 1.0, (const double2*)in, xf));
+    EpilogueF ep;  // s = 1, gamma5
+    OV_TRY(launch_wilson_gather_f32(ctx, xf, yf, ep));
+    return launch_combine_from_f32(ctx, yf, 0.0, nullptr, 0.0, nullptr, 0, (double2*)out);
+}
+
 int ov_set_cg_adaptive(ov_ctx* ctx, int mode) {
     if (!ctx) return OV_EINVAL;
     if (mode < 0 || mode > 2) return fail(ctx, OV_EINVAL, "mode must be 0, 1 or 2");

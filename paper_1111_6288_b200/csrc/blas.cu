@@ -43,6 +43,10 @@ __global__ void su3_defect_kernel(const double2* __restrict__ can, long long nli
             for (int c = 0; c < 3; c++) cmaddc(acc, u[3 * i + c], u[3 * j + c]);
             d = fmax(d, fmax(fabs(acc.x - (i == j ? 1.0 : 0.0)), fabs(acc.y)));
         }
+    if (!(d == d) || isinf(d)) d = INFINITY;                          // fmax drops NaN: a non-finite link must fail the check
+#pragma unroll
+    for (int e = 0; e < 9; e++)
+        if (!isfinite(u[e].x) || !isfinite(u[e].y)) d = INFINITY;
     atomicMax(worst, (unsigned long long)__double_as_longlong(d));   // non-negative doubles order like integers
 }
 
@@ -144,8 +148,8 @@ __global__ void __launch_bounds__(kEwThreads) axpy_kernel(double2 a, const doubl
 }
 
 // z = a x + b y (a, b real); x or y may be null (treated as zero); z may alias x or y
-__global__ void __launch_bounds__(kEwThreads) axpby_kernel(double a, const double2* __restrict__ x, double b,
-                                                           const double2* __restrict__ y, double2* z,
+__global__ void __launch_bounds__(kEwThreads) axpby_kernel(double a, const double2* x, double b,
+                                                           const double2* y, double2* z,   // no __restrict__: z may alias x or y
                                                            long long n) {
     const long long base = (long long)blockIdx.x * (kEwThreads * kEw) + threadIdx.x;
 #pragma unroll

@@ -118,6 +118,12 @@ static double inverse_filter(const Filter& f, double theta_abs) {
 
 using namespace ov;
 
+extern "C" int ov_lanczos_stats(const ov_ctx* ctx, double* out_host) {
+    if (!ctx || !out_host) return OV_EINVAL;
+    for (int i = 0; i < 6; i++) out_host[i] = ctx->lanczos_stats[i];
+    return OV_OK;
+}
+
 extern "C" int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_restarts, int cheb_order, int subspace,
                                    void* V_out_dev, double* lambda_out_host, double* resid_out_host) {
     if (!ctx) return OV_EINVAL;
@@ -197,12 +203,18 @@ extern "C" int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_resta
     int l = 0;            // kept Ritz vectors at the front of W
     double tolB = 0.1 * tol;
     bool refined_filter = false;
+    int widenings = 0;
+    long long filter_applies = 0;
+    const long long launches0 = ctx->launches;
+    ctx->lanczos_stats = {};
     int rc_final = OV_ENOCONV;
     // start vector: W[0] stays (normalised random)
     for (int restart = 0; restart < max_restarts; restart++) {
+        ctx->lanczos_stats = {(double)(restart + 1), (double)filter_applies, 0.0, f.a, (double)widenings, (double)m};
         for (int j = l; j < m; j++) {
             double2* u = W.vec(j + 1);
             OV_TRY(apply_filter(ctx, f, W.vec(j), u, t1, tq));
+            filter_applies++;
             OV_TRY(cgs_pass(ctx, W, j + 1, u, d_C, c));
             double alpha = c[j].x;
             OV_TRY(cgs_pass(ctx, W, j + 1, u, d_C, c));
@@ -234,23 +246,35 @@ extern "C" int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_resta
             zk[i] = make_double2(beta_last * s.x, -beta_last * s.y);   // T[i][keep]
         }
 
+        // restart the Krylov space from the sum of the kept Ritz vectors with a new filter edge
+        auto restart_with_edge = [&](double new_a) -> int {
+            f.a = new_a;
+            std::vector<double2> ones((size_t)keep, make_double2(1.0, 0.0));
+            OV_CUDA(ctx, cudaMemcpyAsync(d_C, ones.data(), keep * sizeof(double2), cudaMemcpyHostToDevice, ctx->stream));
+            OV_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+            OV_TRY(basis_axpy(ctx, W, 1, keep - 1, d_C, W.vec(0)));   // W[0] = sum of the kept Ritz vectors
+            OV_TRY(normalise(W.vec(0), &nrm));
+            std::fill(T.begin(), T.end(), make_double2(0, 0));
+            l = 0;
+            return OV_OK;
+        };
         if (!refined_filter) {
+            // completeness guard: the amplified window [0, f.a) of Q^2 must hold the whole kept set.  If the keep-th Ritz
+            // value is not amplified (|theta| <= 1: it sits in the damped interval, so modes below lambda_k may be hidden
+            // there too), the first guess 4 theta_min was too tight -- widen the window and start again.
+            if (std::fabs(th[kept[keep - 1]]) <= 1.0 + 1e-6 && f.a < 0.9 && widenings < 12) {
+                widenings++;
+                OV_TRY(restart_with_edge(std::min(2.0 * f.a, 0.9)));
+                continue;
+            }
             // tighten the filter edge to just above the kept set, restart the Krylov space from the Ritz vectors
             const double xa = inverse_filter(f, std::fabs(th[kept[keep - 1]]));
             refined_filter = true;
             if (xa > 0 && xa < f.a) {
-                f.a = std::max(xa, 1.0001 * inverse_filter(f, std::fabs(th[kept[k - 1]])));
-                std::vector<double2> ones((size_t)keep, make_double2(1.0, 0.0));
-                OV_CUDA(ctx, cudaMemcpyAsync(d_C, ones.data(), keep * sizeof(double2), cudaMemcpyHostToDevice, ctx->stream));
-                OV_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-                OV_TRY(basis_axpy(ctx, W, 1, keep - 1, d_C, W.vec(0)));   // W[0] = sum of the kept Ritz vectors
-                OV_TRY(normalise(W.vec(0), &nrm));
-                std::fill(T.begin(), T.end(), make_double2(0, 0));
-                l = 0;
+                OV_TRY(restart_with_edge(std::max(xa, 1.0001 * inverse_filter(f, std::fabs(th[kept[k - 1]])))));
                 continue;
             }
         }
-
         if (conv) {
             // Rayleigh-Ritz in Q on span(W[0..keep)): M = Y^+ Q Y
             std::vector<double2> M((size_t)keep * keep), SM;
@@ -327,6 +351,10 @@ extern "C" int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_resta
         }
         l = keep;
     }
+    ctx->lanczos_stats[1] = (double)filter_applies;
+    ctx->lanczos_stats[2] = (double)(ctx->launches - launches0);
+    ctx->lanczos_stats[3] = f.a;
+    ctx->lanczos_stats[4] = (double)widenings;
     OV_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     if (rc_final != OV_OK) return fail(ctx, OV_ENOCONV, "lanczos: residual above tol after %d restarts", max_restarts);
     return OV_OK;

@@ -102,6 +102,9 @@ extern "C" int ov_multishift_cg(ov_ctx* ctx, const double* masses_host, int nmas
     std::vector<double> trunc;
     if (ctx->cg_adaptive) {
         double x_lo = ctx->eps;
+        // The polynomial only has to be accurate on the spectrum the small space does not cover.  Precondition (include/ov.h,
+        // ov_set_cg_adaptive): the caller's small space is COMPLETE below max|lambda_i|, i.e. it holds every mode of Q with
+        // |lambda| < max|lambda_i| (what ov_lanczos_lowmodes returns); then x_lo can move up to ~lambda_k^2.
         if (ctx->k > 0) {
             double lmax = 0.0;
             for (double l : ctx->lambda) lmax = std::max(lmax, std::fabs(l));
@@ -133,6 +136,10 @@ extern "C" int ov_multishift_cg(ov_ctx* ctx, const double* masses_host, int nmas
         if (s0 != 0.0) OV_TRY(launch_axpy(ctx, make_double2(s0, 0.0), p[0], q));
         double2 pq;
         OV_TRY(dot_host(ctx, p[0], q, &pq));
+        // breakdown guard: (p, (A + s0) p) must be positive and finite for a positive definite A; an inexact (reduced
+        // order / fp32) operator or NaN input would otherwise poison every shift silently
+        if (!(pq.x > 0.0) || !std::isfinite(pq.x) || !std::isfinite(rr))
+            return fail(ctx, OV_ENOCONV, "multi-shift CG breakdown at iteration %d: (p, A p) = %g, |r|^2 = %g", it, pq.x, rr);
         const double a = rr / pq.x;
         for (int j = 0; j < nmass; j++) {
             const double s = sig[ord[j]] - s0;

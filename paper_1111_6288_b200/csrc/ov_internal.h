@@ -2,6 +2,7 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <array>
 #include <cstdarg>
 #include <cstdio>
 #include <string>
@@ -67,6 +68,7 @@ struct ov_ctx {
     float2* gauge_f = nullptr; // fp32 copy of the links, same layout (made on first use by the adaptive CG)
     int dslash_variant = 0;
     std::vector<int> cg_orders;  // order used at each iteration of the last adaptive CG (negative: fp32 sweep)
+    std::array<double, 6> lanczos_stats{};  // last ov_lanczos_lowmodes: restarts, filter applies, launches, edge a, widenings, m
     int cg_adaptive = 0;  // ov_set_cg_adaptive: 0 off, 1 reduced orders, 2 reduced orders + fp32 sweeps
     int flip = 0;  // block order of the next Wilson launch (alternates)
     bool blocked = false;  // layout of spinors and links (see spinor_base)
@@ -136,6 +138,7 @@ int gauge_su3_defect(ov_ctx* ctx, const double2* canonical, double* defect);
 int launch_pack(ov_ctx* ctx, const double2* canonical, double2* abi);
 int launch_unpack(ov_ctx* ctx, const double2* abi, double2* canonical);
 int launch_wilson(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep);
+int effective_variant(const ov_ctx* ctx);  // 1 = gather, 2 = TMA-staged: what launch_wilson picks for this context
 int launch_wilson_gather(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep);
 // batched: nrhs consecutive ABI spinors (stride 12 V) in in/out and in every epilogue operand
 int launch_wilson_batch(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep, int nrhs);

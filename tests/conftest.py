@@ -28,3 +28,25 @@ def load_golden(name="paper_values.txt"):
 @pytest.fixture(scope="session")
 def golden():
     return load_golden()
+
+
+# Observed parity errors: tests call record_parity(...); the numbers are printed in the terminal summary (also with -q and
+# for passing tests), so the driver's log records what was actually measured, not only that it was under the gate.
+PARITY_LOG = []
+
+
+def record_parity(name, observed, gate):
+    PARITY_LOG.append((name, float(observed), float(gate)))
+
+
+@pytest.fixture(scope="session")
+def parity_log():
+    return record_parity
+
+
+def pytest_terminal_summary(terminalreporter):
+    if not PARITY_LOG:
+        return
+    terminalreporter.write_line("observed parity (name: observed <= gate)")
+    for name, obs, gate in PARITY_LOG:
+        terminalreporter.write_line(f"  {name}: {obs:.3e} <= {gate:.1e}")

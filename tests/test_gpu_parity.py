@@ -49,10 +49,6 @@ def to_host(op, x):
     return op.unpack_spinor(x).cpu().numpy()
 
 
-def variants(op_dims):
-    return [1, 2]
-
-
 # ------------------------------------------------------------------------------------------ layout
 def test_pack_unpack_roundtrip(ovp):
     dims = (4, 2, 6, 8)
@@ -247,6 +243,39 @@ def test_lanczos_4x4_vs_dense(ovp, cfg0):
         assert np.linalg.norm(r.ravel()) <= 1e-8
     G = Vh.reshape(k, -1).conj() @ Vh.reshape(k, -1).T
     assert np.max(np.abs(G - np.eye(k))) <= 1e-10
+
+
+# ------------------------------------------------------------------------------------------ T-small on the GPU
+def test_small_space_needed_on_gpu(ovp, parity_log):
+    """The oracle's pin P11 run through the CUDA path: sqrt(eps) sits between q_k and q_{k+1}, the source lives mostly in
+    the k low modes, so without the small space the polynomial alone is wrong at O(1) on them, and with it the result is
+    within delta of the exact dense sign -- a wrong sign(lambda_i), a dropped v_i or a mis-ordered coefficient fails here."""
+    dims = (4, 4, 4, 4)
+    U = wl.su3_links(dims, 0.5, 77)
+    w, Zv, _, _ = dense.eig_hw(dims, KAPPA, U)
+    q = np.sort(np.abs(w)) / NORM
+    k = 10
+    se = 0.5 * (q[k - 1] + q[k])
+    coef = ch.cheb_coeffs(60, se * se)
+    x0 = wl.gaussian_source(dims, 78)
+    V, lam = dense.lowest_modes(w, Zv, NORM, k, x0.shape)
+    assert (lam > 0).any() and (lam < 0).any()              # both signs present
+    x = x0 * 1e-3 + np.tensordot(np.arange(1, k + 1) * (1 + 0.5j), V, axes=(0, 0))
+    exact = dense.exact_sign_apply(w, Zv, x)
+    d = ch.delta_measured(coef, se * se)
+    op = make(ovp, dims, U)
+    op.set_polynomial(coef, se * se, NORM)
+    dx = to_dev(op, x)
+    without = to_host(op, op.apply_sign(dx))
+    op.set_smallspace(to_dev(op, V), lam)
+    with_k = to_host(op, op.apply_sign(dx))
+    e_with, e_without = rel(with_k, exact), rel(without, exact)
+    parity_log("4^4 T-small on the GPU: sign with small space vs exact dense sign", e_with, d)
+    parity_log("4^4 T-small on the GPU: oracle vs GPU with small space", rel(with_k, oracle.sign(dims, KAPPA, U, coef, se * se, NORM, V, lam, x)), TOL_DOV)
+    assert e_with <= d
+    assert e_without > 3 * e_with
+    assert rel(with_k, oracle.sign(dims, KAPPA, U, coef, se * se, NORM, V, lam, x)) <= TOL_DOV
+    assert rel(without, oracle.sign(dims, KAPPA, U, coef, se * se, NORM, None, None, x)) <= TOL_DOV
 
 
 # ------------------------------------------------------------------------------------------ adaptive CG (PAPER.md:87)

@@ -334,3 +334,38 @@ def test_multishift_cg_on_overlap(cfg0):
     sig = [sigma_of_mass(m) for m in masses]
     xs, it, res = multishift_cg(A, sig, c["x"], 1e-9, 200)
     assert it < 200 and np.all(res < 1e-8)
+
+
+# ---------------------------------------------------------------- stored low modes of the 8^4 completeness pin
+def test_golden_lowmodes_file_is_this_operator():
+    """tests/golden/lowmodes_8x8x8x8.txt is written by tests/golden/make_lowmodes_golden.py (oracle H_w + ARPACK, minutes).
+    Cheap consistency check that the file belongs to this operator, seed and norm: a plain 150-step Lanczos on Q^2 with
+    the oracle's H_w gives Ritz values that bound the spectrum from inside (theta_min >= lambda_1^2, theta_max <= 1) and,
+    at the well-separated upper end, has converged; the lower end must sit within the stored cluster."""
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "lowmodes_8x8x8x8.txt")
+    gold = np.array([float(l) for l in open(path) if l.strip() and not l.startswith("#")])
+    assert len(gold) == 40 and np.all(np.diff(np.abs(gold)) > 0) and (gold > 0).any() and (gold < 0).any()
+    dims = (8, 8, 8, 8)
+    U = wl.su3_links(dims, 0.5, wl.gauge_seed(7))
+    shape = (8, 8, 8, 8, 4, 3)
+    q = lambda v: oracle.hw(dims, KAPPA, U, v.reshape(shape)).reshape(-1) / NORM
+    rng = np.random.default_rng(3)
+    v = rng.standard_normal(12 * 4096) + 1j * rng.standard_normal(12 * 4096)
+    v /= np.linalg.norm(v)
+    m = 150
+    Vk = np.zeros((m, v.size), dtype=np.complex128)
+    al, be = np.zeros(m), np.zeros(m)
+    for j in range(m):
+        Vk[j] = v
+        w = q(q(v))
+        al[j] = np.vdot(v, w).real
+        w -= Vk[:j + 1].T @ (Vk[:j + 1].conj() @ w)       # full reorthogonalisation
+        w -= Vk[:j + 1].T @ (Vk[:j + 1].conj() @ w)
+        be[j] = np.linalg.norm(w)
+        v = w / be[j]
+    Tm = np.diag(al) + np.diag(be[:-1], 1) + np.diag(be[:-1], -1)
+    th = np.linalg.eigvalsh(Tm)
+    assert th[0] >= gold[0] ** 2 * (1 - 1e-9)             # variational: no Ritz value below the lowest eigenvalue
+    assert th[0] <= gold[-1] ** 2                          # ... and the Krylov space has reached the stored cluster
+    assert th[-1] <= 1.0                                   # norm = 1 + 8 kappa bounds the spectrum of Q
