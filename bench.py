@@ -43,7 +43,8 @@ def parse_args():
     ap.add_argument("--order", type=int, default=None, help="override the Chebyshev order (testing only)")
     ap.add_argument("--k", type=int, default=None, help="override the number of low modes (testing only)")
     ap.add_argument("--recon", type=int, default=18, choices=[18, 12])
-    ap.add_argument("--variant", type=int, default=0, help="dslash kernel variant (0 = automatic)")
+    ap.add_argument("--variant", type=int, default=0, help="dslash kernel variant (0 = automatic, 1 = gather, 2 = TMA-staged)")
+    ap.add_argument("--layout", default="auto", choices=["auto", "blocked", "planes"], help="spinor/link layout (ov_options.layout)")
     ap.add_argument("--modes-file", default=None,
                     help="torch file with the low modes {V, lam}: loaded if present, else written after Lanczos")
     ap.add_argument("--lanczos-order", type=int, default=100, help="Chebyshev filter order (paper: 100)")
@@ -319,7 +320,7 @@ def run_b200(args):
     t0 = time.perf_counter()
     U = wl.su3_links(cfg.dims, cfg.spread, wl.gauge_seed(cfg.index))
     log(f"links generated in {time.perf_counter() - t0:.1f} s")
-    op = ovp.Overlap(cfg.dims, cfg.kappa, U, recon=args.recon)
+    op = ovp.Overlap(cfg.dims, cfg.kappa, U, recon=args.recon, layout=args.layout)
     if args.variant:
         op.set_dslash_variant(args.variant)
     coef = ovp.chebyshev_coeffs(order, cfg.eps)
@@ -525,6 +526,7 @@ def finish(args, cfg, order, k, V_sites, world, ms, value, launches, tim, e2e, h
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_name(cfg, order, k), "recon": args.recon, "parallelism": f"replicas x{world}",
+                   "dslash_variant": variant_used, "layout": args.layout,
                    "l2": "inputs larger than L2 (gauge 510 MB + 17 GB of low modes stream every step)",
                    "low_modes": f"GPU Lanczos, max residual {resid:.1e}, {lanczos_s:.0f} s (untimed setup)" if k else "none"},
         "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu, "cg_time_to_solution": cg, "batched": batched, "recon12": recon12,
@@ -545,8 +547,9 @@ def run_kernels(args):
     cfg = wl.CONFIGS[args.config]
     V = wl.volume(cfg.dims)
     U = wl.su3_links(cfg.dims, cfg.spread, wl.gauge_seed(cfg.index))
-    op = ovp.Overlap(cfg.dims, cfg.kappa, U, recon=18)
+    op = ovp.Overlap(cfg.dims, cfg.kappa, U, recon=18)              # automatic layout and kernel choice
     op12 = ovp.Overlap(cfg.dims, cfg.kappa, U, recon=12)
+    opb = ovp.Overlap(cfg.dims, cfg.kappa, U, recon=18, layout="blocked") if V % 32 == 0 else None   # gather kernel's best layout
     peak, peak_src = measured_peak()
     k = 16  # a small stand-in basis is enough to time the projector kernels per vector
     xs = [op.pack_spinor(torch.from_numpy(wl.gaussian_source(cfg.dims, 100 + j)).cuda()) for j in range(2)]
@@ -580,9 +583,21 @@ def run_kernels(args):
 
     out = torch.empty_like(x)
     torch.cuda.cudart().cudaProfilerStart()
-    add("wilson_gather<18> H_w (ov_apply_hw)", 960.0 * V, lambda: op.apply_hw(x, out))
-    add("wilson_gather<18> hop only (ov_dslash)", 960.0 * V, lambda: op.dslash(x, out))
-    add("wilson_gather<12> H_w (recon 12)", 768.0 * V, lambda: op12.apply_hw(x, out))
+    vname = {1: "wilson_gather", 2: "wilson_tma"}
+    for v in ((2, 1) if op.dslash_variant == 2 else (1,)):
+        op.set_dslash_variant(v)
+        op12.set_dslash_variant(v)
+        lay = "blocked" if op.spinor_layout == 1 else "planes"
+        add(f"{vname[v]}<18> H_w (ov_apply_hw, {lay} layout)", 960.0 * V, lambda: op.apply_hw(x, out))
+        add(f"{vname[v]}<18> hop only (ov_dslash, {lay} layout)", 960.0 * V, lambda: op.dslash(x, out))
+        add(f"{vname[v]}<12> H_w (recon 12, {lay} layout)", 768.0 * V, lambda: op12.apply_hw(x, out))
+        add(f"{vname[v]}<18> D_ov reduced, order 8, fp64 sweep (17 Wilson launches + projector), {lay} layout", 0.0,
+            lambda: op.apply_dov_reduced(0.0, x, 8, False, out), 10)
+    op.set_dslash_variant(0)
+    op12.set_dslash_variant(0)
+    if opb is not None and op.spinor_layout != 1:
+        xb_, ob_ = opb.pack_spinor(can), opb.new_spinor()
+        add("wilson_gather<18> H_w (ov_apply_hw, blocked layout)", 960.0 * V, lambda: opb.apply_hw(xb_, ob_))
     add("wilson_gather<18> batched, 4 rhs per launch", (4 * 384.0 + 576.0) * V, lambda: op.apply_hw(x4, y4), 20)
     add("axpy (ov_blas_axpy)", 3 * S, lambda: op.blas_axpy(0.5 + 0.25j, x, out))
     add("scale (ov_blas_scale)", 2 * S, lambda: op.blas_scale(1.0, out))
@@ -591,7 +606,6 @@ def run_kernels(args):
     add("unpack (ov_unpack_spinor)", 2 * S, lambda: op.unpack_spinor(x))
     add(f"projector k={k}: multi_dot + coef + multi_axpy<2> (ov_project, incl. host copy of c)", (2 * k + 4) * S,
         lambda: op.project(x), 20)
-    add("D_ov reduced, order 8, fp64 sweep (17 Wilson launches + projector)", 0.0, lambda: op.apply_dov_reduced(0.0, x, 8, False, out), 10)
     add("D_ov reduced, order 8, fp32 sweep (17 fp32 Wilson launches + projector + conversions)", 0.0,
         lambda: op.apply_dov_reduced(0.0, x, 8, True, out), 10)
     torch.cuda.cudart().cudaProfilerStop()

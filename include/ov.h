@@ -62,6 +62,21 @@ typedef struct ov_ctx ov_ctx;
  * cuda_stream: a cudaStream_t (NULL = legacy default stream).                                        */
 int ov_create(ov_ctx** out, const int dims[4], double kappa, const void* gauge_dev, int recon,
               void* cuda_stream);
+/* ov_create_ex: the same with options (NULL or all-zero = ov_create).
+ *   layout      0 automatic (planes when the TMA-staged Wilson kernel applies, i.e. X % 8 == 0, Y % 4 == 0, Z % 4 == 0;
+ *                 else blocked when V % 32 == 0; else planes), 1 blocked (needs V % 32 == 0), 2 planes.
+ *   t_boundary  what the hop between t = T-1 and t = 0 is multiplied by: OV_BC_ANTIPERIODIC (-1, the default of this
+ *               library: north_star, reading G11), OV_BC_PERIODIC (+1), OV_BC_OPEN (0: no hop across the
+ *               boundary, the Dirichlet condition in time of PAPER.md:104).  Dirichlet walls in a space direction are
+ *               zero links on the wall (ov_background_field writes them); recon = 18 takes such links.            */
+enum { OV_BC_ANTIPERIODIC = 0, OV_BC_PERIODIC = 1, OV_BC_OPEN = 2 };
+typedef struct ov_options {
+    int layout;
+    int t_boundary;
+    int reserved[6]; /* must be zero */
+} ov_options;
+int ov_create_ex(ov_ctx** out, const int dims[4], double kappa, const void* gauge_dev, int recon,
+                 void* cuda_stream, const ov_options* options);
 void ov_destroy(ov_ctx* ctx);
 const char* ov_last_error(const ov_ctx* ctx);
 size_t ov_spinor_bytes(const ov_ctx* ctx); /* 192 * V */
@@ -75,9 +90,11 @@ long long ov_launch_count(const ov_ctx* ctx);
  *                 ms inside the small-space projector, kernel launches in it }  and resets the accumulators. */
 int ov_timing_enable(ov_ctx* ctx, int on);
 int ov_timing_read(ov_ctx* ctx, double* out_host);
-/* selects the dslash kernel: 0 = automatic, 1 = gather (one thread per site, operands through L1/L2).  2 is reserved
- * for a shared-memory staged kernel; the staged designs measured so far were slower than the gather kernel (DESIGN.md
- * section 10), none ships, and the call returns OV_EINVAL. */
+/* selects the Wilson kernel of single-right-hand-side launches: 0 = automatic (the TMA-staged kernel where it applies,
+ * see DESIGN.md section 10), 1 = gather (one thread per site, operands through L1/L2; every shape and layout),
+ * 2 = TMA-staged (persistent warp-specialised kernel: cp.async.bulk.tensor into shared-memory rings, mbarrier
+ * producer/consumer; needs the planes layout and X % 8 == 0, Y % 4 == 0, Z % 4 == 0, else OV_EINVAL).  Both give
+ * bit-identical results. */
 int ov_set_dslash_variant(ov_ctx* ctx, int variant);
 /* the variant single-right-hand-side Wilson launches of this context actually use (1 or 2; never 0) */
 int ov_get_dslash_variant(const ov_ctx* ctx);

@@ -20,7 +20,7 @@ _CODES = {1: "OV_EINVAL", 2: "OV_ENOMEM", 3: "OV_ECUDA", 4: "OV_ESTATE", 5: "OV_
 
 # every symbol include/ov.h declares (tests check that the library exports all of them)
 SYMBOLS = [
-    "ov_create", "ov_destroy", "ov_last_error", "ov_spinor_bytes", "ov_volume", "ov_spinor_layout", "ov_launch_count",
+    "ov_create", "ov_create_ex", "ov_destroy", "ov_last_error", "ov_spinor_bytes", "ov_volume", "ov_spinor_layout", "ov_launch_count",
     "ov_timing_enable", "ov_timing_read",
     "ov_set_dslash_variant", "ov_get_dslash_variant", "ov_pack_spinor", "ov_unpack_spinor", "ov_dslash", "ov_apply_hw",
     "ov_chebyshev_coeffs", "ov_set_polynomial", "ov_set_smallspace", "ov_project", "ov_apply_sign",
@@ -95,7 +95,10 @@ class Overlap:
     """One ov_ctx.  Spinor arguments are torch complex128 CUDA tensors in the ABI layout [nrhs?][12][V]
     unless a method says "canonical" ([T][Z][Y][X][4][3])."""
 
-    def __init__(self, dims, kappa, gauge, recon=18, stream=None):
+    LAYOUTS = {"auto": 0, "blocked": 1, "planes": 2}
+    BOUNDARIES = {"antiperiodic": 0, "periodic": 1, "open": 2}
+
+    def __init__(self, dims, kappa, gauge, recon=18, stream=None, layout="auto", t_boundary="antiperiodic"):
         if not torch.cuda.is_available():
             raise OvError(OV_ECUDA, "no CUDA device: this library has no CPU fallback")
         self.lib = load_library()
@@ -108,8 +111,9 @@ class Overlap:
         self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         self._ctx = ctypes.c_void_p()
         cdims = (ctypes.c_int * 4)(*self.dims)
-        rc = self.lib.ov_create(ctypes.byref(self._ctx), cdims, ctypes.c_double(kappa), _ptr(gauge.contiguous()),
-                                ctypes.c_int(recon), ctypes.c_void_p(self.stream.cuda_stream))
+        opt = (ctypes.c_int * 8)(self.LAYOUTS[layout], self.BOUNDARIES[t_boundary], 0, 0, 0, 0, 0, 0)   # struct ov_options
+        rc = self.lib.ov_create_ex(ctypes.byref(self._ctx), cdims, ctypes.c_double(kappa), _ptr(gauge.contiguous()),
+                                   ctypes.c_int(recon), ctypes.c_void_p(self.stream.cuda_stream), opt)
         if rc != OV_OK:
             raise OvError(rc, "ov_create failed")
         self._keepalive = None

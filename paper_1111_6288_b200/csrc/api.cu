@@ -57,9 +57,16 @@ int ensure_reduction_buffers(ov_ctx* ctx, size_t partial_elems, size_t result_el
     return OV_OK;
 }
 
-int effective_variant(const ov_ctx* ctx) { return 1; }
+static bool tma_usable(const ov_ctx* ctx) { return !ctx->blocked && tma_eligible(ctx->lat); }
+
+int effective_variant(const ov_ctx* ctx) {
+    if (ctx->dslash_variant == 1) return 1;
+    if (ctx->dslash_variant == 2) return 2;
+    return tma_usable(ctx) ? 2 : 1;
+}
 
 int launch_wilson(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep) {
+    if (effective_variant(ctx) == 2) return launch_wilson_tma(ctx, in, out, ep);
     return launch_wilson_gather(ctx, in, out, ep);
 }
 
@@ -105,7 +112,17 @@ using namespace ov;
 extern "C" {
 
 int ov_create(ov_ctx** out, const int dims[4], double kappa, const void* gauge_dev, int recon, void* cuda_stream) {
+    return ov_create_ex(out, dims, kappa, gauge_dev, recon, cuda_stream, nullptr);
+}
+
+int ov_create_ex(ov_ctx** out, const int dims[4], double kappa, const void* gauge_dev, int recon, void* cuda_stream,
+                 const ov_options* options) {
     if (!out) return OV_EINVAL;
+    ov_options opt{};
+    if (options) opt = *options;
+    if (opt.layout < 0 || opt.layout > 2 || opt.t_boundary < 0 || opt.t_boundary > 2) return OV_EINVAL;
+    for (int r : opt.reserved)
+        if (r != 0) return OV_EINVAL;
     *out = nullptr;
     if (!dims || !gauge_dev) return OV_EINVAL;
     if (recon != 18 && recon != 12) return OV_EINVAL;
@@ -119,9 +136,9 @@ int ov_create(ov_ctx** out, const int dims[4], double kappa, const void* gauge_d
     ctx->lat.V = (long long)dims[0] * dims[1] * dims[2] * dims[3];
     ctx->kappa = kappa;
     ctx->recon = recon;
-#ifndef OV_FORCE_PLANES
-    ctx->blocked = (ctx->lat.V % 32) == 0;
-#endif
+    if (opt.layout == 1 && ctx->lat.V % 32 != 0) { delete ctx; return OV_EINVAL; }
+    ctx->blocked = opt.layout == 1 || (opt.layout == 0 && ctx->lat.V % 32 == 0 && !tma_eligible(ctx->lat));
+    ctx->t_phase = opt.t_boundary == OV_BC_PERIODIC ? 1.0 : opt.t_boundary == OV_BC_OPEN ? 0.0 : -1.0;
     ctx->stream = (cudaStream_t)cuda_stream;
     const size_t gbytes = gauge_elems(ctx->lat.V, recon) * sizeof(double2);
     cudaError_t e = cudaMalloc(&ctx->gauge, gbytes);
@@ -157,6 +174,7 @@ void ov_destroy(ov_ctx* ctx) {
     cudaFree(ctx->host_stage_abi);
     cudaFree(ctx->host_stage_out);
     for (auto e : ctx->ev_pool) cudaEventDestroy(e);
+    tma_state_free(ctx);
     delete ctx;
 }
 
@@ -194,7 +212,8 @@ int ov_timing_read(ov_ctx* ctx, double* out_host) {
 int ov_set_dslash_variant(ov_ctx* ctx, int variant) {
     if (!ctx) return OV_EINVAL;
     if (variant < 0 || variant > 2) return fail(ctx, OV_EINVAL, "variant must be 0, 1 or 2");
-    if (variant == 2) return fail(ctx, OV_EINVAL, "no shared-memory staged Wilson kernel in this build (DESIGN.md section 10)");
+    if (variant == 2 && !tma_usable(ctx))
+        return fail(ctx, OV_EINVAL, "the TMA-staged Wilson kernel needs the planes layout and X %% 8 == Y %% 4 == Z %% 4 == 0");
     ctx->dslash_variant = variant;
     return OV_OK;
 }

@@ -66,7 +66,9 @@ struct ov_ctx {
     cudaStream_t stream = nullptr;
     double2* gauge = nullptr;  // see gauge_index()
     float2* gauge_f = nullptr; // fp32 copy of the links, same layout (made on first use by the adaptive CG)
-    int dslash_variant = 0;
+    int dslash_variant = 0;    // ov_set_dslash_variant: 0 automatic, 1 gather, 2 TMA-staged
+    double t_phase = -1.0;     // factor on the hop across the t boundary (ov_options::t_boundary)
+    void* tma_state = nullptr; // tensor maps and schedule of the TMA-staged kernel (wilson_tma.cu)
     std::vector<int> cg_orders;  // order used at each iteration of the last adaptive CG (negative: fp32 sweep)
     std::array<double, 6> lanczos_stats{};  // last ov_lanczos_lowmodes: restarts, filter applies, launches, edge a, widenings, m
     int cg_adaptive = 0;  // ov_set_cg_adaptive: 0 off, 1 reduced orders, 2 reduced orders + fp32 sweeps
@@ -140,6 +142,9 @@ int launch_unpack(ov_ctx* ctx, const double2* abi, double2* canonical);
 int launch_wilson(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep);
 int effective_variant(const ov_ctx* ctx);  // 1 = gather, 2 = TMA-staged: what launch_wilson picks for this context
 int launch_wilson_gather(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep);
+int launch_wilson_tma(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep);   // variant 2 (wilson_tma.cu)
+bool tma_eligible(const Lattice& lat);
+void tma_state_free(ov_ctx* ctx);
 // batched: nrhs consecutive ABI spinors (stride 12 V) in in/out and in every epilogue operand
 int launch_wilson_batch(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep, int nrhs);
 int launch_wilson_gather_f32(ov_ctx* ctx, const float2* in, float2* out, const EpilogueF& ep);  // needs ctx->gauge_f

@@ -23,6 +23,7 @@ struct GatherArgs {
     int X, Y, Z, T;
     long long V;
     double kappa;
+    double tphase;         // factor on the hop across the t boundary: -1 antiperiodic, +1 periodic, 0 open
     int reverse;
     int nrb;               // rhs groups per site block (batched launch): block id = site_block * nrb + rhs_group
     long long rhs_stride;  // elements between consecutive right-hand sides in in/out/A1..A3
@@ -123,8 +124,8 @@ wilson_gather_kernel(GatherArgs<C> a) {
         const bool wp = (t + 1 == a.T), wm = (t == 0);
         const long long ip = wp ? i - (a.T - 1) * sT : i + sT;
         const long long im = wm ? i + (a.T - 1) * sT : i - sT;
-        hop<3, -1, RECON, BL>(acc, a, ip, i, wp ? (R)-1 : (R)1);  // antiperiodic in time
-        hop<3, +1, RECON, BL>(acc, a, im, im, wm ? (R)-1 : (R)1);
+        hop<3, -1, RECON, BL>(acc, a, ip, i, wp ? (R)a.tphase : (R)1);  // boundary in time (default antiperiodic)
+        hop<3, +1, RECON, BL>(acc, a, im, im, wm ? (R)a.tphase : (R)1);
     }
 
     const EpilogueT<C>& ep = a.ep;
@@ -185,13 +186,10 @@ static int launch_gather_t(ov_ctx* ctx, const C* gauge, const C* in, C* out, con
     a.X = ctx->lat.X; a.Y = ctx->lat.Y; a.Z = ctx->lat.Z; a.T = ctx->lat.T;
     a.V = ctx->lat.V;
     a.kappa = ctx->kappa;
+    a.tphase = ctx->t_phase;
     a.ep = ep;
-#ifdef OV_NO_ALTERNATE
-    a.reverse = 0;
-#else
     a.reverse = ctx->flip;
     ctx->flip ^= 1;
-#endif
     const int threads = GatherShape<C>::threads;
     const unsigned blocks = (unsigned)((a.V + threads - 1) / threads) * (unsigned)a.nrb;
     const dim3 bdim(threads, rb);

@@ -220,6 +220,7 @@ def cfg2(ovp):
     op.set_polynomial(ovp.chebyshev_coeffs(cfg.order, cfg.eps), cfg.eps, cfg.norm)
     V, lam, res, ok = op.lanczos_lowmodes(cfg.k, tol=1e-8, max_restarts=60, cheb_order=100)
     assert ok
+    op.set_smallspace(V, lam)
     return dict(cfg=cfg, U=U, op=op, V=V, lam=lam, Vh=host(op, V))
 
 

@@ -74,7 +74,8 @@ def test_pack_unpack_roundtrip(ovp):
 # ------------------------------------------------------------------------------------------ Wilson kernel
 @pytest.mark.parametrize("dims,spread", [((4, 4, 4, 4), 0.3), ((4, 2, 6, 8), 0.6), ((8, 8, 8, 16), 0.5),
                                          ((24, 4, 4, 2), 0.8), ((6, 10, 2, 4), 0.4), ((6, 6, 2, 6), 0.5),
-                                         ((2, 2, 2, 2), 0.7)])
+                                         ((2, 2, 2, 2), 0.7), ((8, 4, 4, 3), 0.6), ((16, 8, 4, 6), 0.7),
+                                         ((8, 12, 8, 5), 0.5)])
 @pytest.mark.parametrize("recon", [18, 12])
 def test_dslash_and_hw_vs_oracle(ovp, dims, spread, recon):
     U = wl.su3_links(dims, spread, wl.gauge_seed(1))
@@ -83,20 +84,26 @@ def test_dslash_and_hw_vs_oracle(ovp, dims, spread, recon):
     ref_hop = np.stack([oracle.wilson_hop(dims, U, v) for v in x])
     ref_hw = np.stack([oracle.hw(dims, KAPPA, U, v) for v in x])
     op = make(ovp, dims, U, recon)
-    tested = 0
-    for variant in (1, 2):
-        try:
-            op.set_dslash_variant(variant)
-        except ovp.OvError:
-            continue
-        tested += 1
+    X, Y, Z, T = dims
+    tma = X % 8 == 0 and Y % 4 == 0 and Z % 4 == 0         # the shapes the TMA-staged kernel (variant 2) takes
+    assert op.dslash_variant == (2 if tma else 1)           # ... and the automatic choice
+    results = {}
+    for variant in ((1, 2) if tma else (1,)):
+        op.set_dslash_variant(variant)
         d = to_dev(op, x)
-        assert rel(to_host(op, op.dslash(d)), ref_hop) <= TOL_HW
-        got = to_host(op, op.apply_hw(d))
-        assert rel(got, ref_hw) <= TOL_HW
+        hop = to_host(op, torch.stack([op.dslash(d[j]) for j in range(nsrc)]))   # single-rhs launches: the chosen variant
+        got = to_host(op, torch.stack([op.apply_hw(d[j]) for j in range(nsrc)]))
+        assert rel(hop, ref_hop) <= TOL_HW
         for j in range(nsrc):
             assert rel(got[j], ref_hw[j]) <= TOL_HW
-    assert tested >= 1
+        results[variant] = (hop, got)
+        # the batched launch (always the gather kernel) agrees too
+        assert rel(to_host(op, op.apply_hw(d)), ref_hw) <= TOL_HW
+    if tma:   # same arithmetic in the same order: the two kernels agree to the last bit
+        assert np.array_equal(results[1][0], results[2][0]) and np.array_equal(results[1][1], results[2][1])
+    if not tma:
+        with pytest.raises(ovp.OvError):
+            op.set_dslash_variant(2)
 
 
 def test_hw_rejects_aliasing_and_bad_args(ovp):
@@ -352,6 +359,38 @@ def test_timing_hooks_and_launch_count(ovp, cfg0):
     assert op.launch_count - l0 == 3 * (2 * n + 1 + 4 + 1)      # + projector (4) + the b_n = c_n x axpby
     with pytest.raises(ovp.OvError):
         op.set_dslash_variant(2)
+
+
+# ------------------------------------------------------------------------------------------ TMA-staged kernel in the sweep
+@pytest.mark.parametrize("recon", [18, 12])
+def test_tma_variant_sign_and_dov_vs_oracle(ovp, recon):
+    """The Clenshaw sweep through the TMA-staged kernel (every epilogue form: 0-3 fused axpy operands) on a lattice of
+    several pencils and time segments with a ragged slice count, against the oracle and against the gather kernel."""
+    dims = (16, 8, 4, 6)
+    U = wl.su3_links(dims, 0.6, 91)
+    x = wl.gaussian_source(dims, 92)
+    se, n = 0.2, 12
+    coef = ovp.chebyshev_coeffs(n, se * se)
+    rng = np.random.default_rng(93)
+    # any orthonormal set serves as a "small space" for parity (both sides get the same V, lambda)
+    A = rng.standard_normal((3, x.size)) + 1j * rng.standard_normal((3, x.size))
+    Qm, _ = np.linalg.qr(A.T)
+    V = np.ascontiguousarray(Qm.T).reshape((3,) + x.shape)
+    lam = np.array([0.05, -0.07, 0.11])
+    op = make(ovp, dims, U, recon)
+    op.set_polynomial(coef, se * se, NORM)
+    op.set_smallspace(to_dev(op, V), lam)
+    dx = to_dev(op, x)
+    ref_s = oracle.sign(dims, KAPPA, U, coef, se * se, NORM, V, lam, x)
+    ref_d = oracle.dov(dims, KAPPA, U, coef, se * se, NORM, V, lam, 0.07, x)
+    out = {}
+    for variant in (2, 1):
+        op.set_dslash_variant(variant)
+        assert op.dslash_variant == variant
+        s, d = to_host(op, op.apply_sign(dx)), to_host(op, op.apply_dov(0.07, dx))
+        assert rel(s, ref_s) <= TOL_DOV and rel(d, ref_d) <= TOL_DOV
+        out[variant] = (s, d)
+    assert np.array_equal(out[1][0], out[2][0]) and np.array_equal(out[1][1], out[2][1])
 
 
 # ------------------------------------------------------------------------------------------ links that are not SU(3)
