@@ -67,13 +67,26 @@ int ov_create(ov_ctx** out, const int dims[4], double kappa, const void* gauge_d
  *                 else blocked when V % 32 == 0; else planes), 1 blocked (needs V % 32 == 0), 2 planes.
  *   t_boundary  what the hop between t = T-1 and t = 0 is multiplied by: OV_BC_ANTIPERIODIC (-1, the default of this
  *               library: north_star, reading G11), OV_BC_PERIODIC (+1), OV_BC_OPEN (0: no hop across the
- *               boundary, the Dirichlet condition in time of PAPER.md:104).  Dirichlet walls in a space direction are
- *               zero links on the wall (ov_background_field writes them); recon = 18 takes such links.            */
+ *               boundary, the Dirichlet condition in time of PAPER.md:104).
+ *   wall_mask   bit mu (mu = 0, 1, 2 = x, y, z) set: Dirichlet wall in that space direction ("Dirichlet
+ *               boundary conditions both in the direction of the applied electric field and time"): the links
+ *               U_mu at coordinate d_mu - 1 are zero in the library's copy of the gauge field, so no hop connects
+ *               coordinate d_mu - 1 and 0.  (Bit 3 is not used: the time direction is t_boundary.)
+ *   field       0 = no background field; 1, 2, 3 = constant electric field along x, y, z (eq. 4.1
+ *               "U_mu -> exp(-i q A_mu) U_mu"), in the gauge A_t(x) = E (x_dir - field_origin), other components zero
+ *               (reading G19: the paper does not fix the gauge): the library's copy of every t link is
+ *               multiplied by exp(-i field_qE (x_dir - field_origin)), field_qE = q E in lattice units.  The links
+ *               are then U(3), so field != 0 needs recon = 18 (OV_EINVAL otherwise); with recon = 12 the SU(3) check
+ *               applies to the caller's links, walls are allowed.                                                  */
 enum { OV_BC_ANTIPERIODIC = 0, OV_BC_PERIODIC = 1, OV_BC_OPEN = 2 };
 typedef struct ov_options {
     int layout;
     int t_boundary;
-    int reserved[6]; /* must be zero */
+    int wall_mask;
+    int field;
+    int field_origin;
+    int reserved;    /* must be zero */
+    double field_qE;
 } ov_options;
 int ov_create_ex(ov_ctx** out, const int dims[4], double kappa, const void* gauge_dev, int recon,
                  void* cuda_stream, const ov_options* options);

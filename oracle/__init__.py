@@ -21,4 +21,7 @@ from .capi import (  # noqa: F401
     sign,
     dov,
     num_threads,
+    set_boundary,
+    boundary,
+    BC_DEFAULT,
 )

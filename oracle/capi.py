@@ -54,6 +54,31 @@ def _dims(dims):
     return (ctypes.c_int * 4)(*[int(d) for d in dims])
 
 
+BC_DEFAULT = (1.0, 1.0, 1.0, -1.0)   # periodic in space, antiperiodic in time (north_star; G11)
+
+
+def set_boundary(bc=BC_DEFAULT) -> None:
+    """Boundary factor per direction (x, y, z, t) of a hop across the lattice boundary: +1 periodic, -1 antiperiodic,
+    0 Dirichlet/open.  Global state of the C oracle; every operator below uses it."""
+    arr = (ctypes.c_double * 4)(*[float(v) for v in bc])
+    _load().orc_set_boundary(arr)
+
+
+class boundary:
+    """with oracle.boundary((1, 1, 0, 0)): ...   -- sets the boundary factors, restores the default on exit."""
+
+    def __init__(self, bc):
+        self.bc = bc
+
+    def __enter__(self):
+        set_boundary(self.bc)
+        return self
+
+    def __exit__(self, *exc):
+        set_boundary(BC_DEFAULT)
+        return False
+
+
 def gamma(idx: int) -> np.ndarray:
     """gamma_x, gamma_y, gamma_z, gamma_t (idx 0..3) or gamma5 (idx 4) as the oracle uses them."""
     out = np.zeros((4, 4), dtype=np.complex128)

@@ -50,9 +50,19 @@ void orc_gamma(int idx, cplx *out16)
 
 static long nsites(const int *d) { return (long)d[0] * d[1] * d[2] * d[3]; }
 
+/* Boundary factor of a hop that crosses the lattice boundary in direction mu: +1 periodic, -1 antiperiodic,
+ * 0 Dirichlet/open (the hop is removed).  Default = north_star's: periodic in space, antiperiodic in time
+ * (reading G11).  PAPER.md:104 "we use Dirichlet boundary conditions both in the direction of the
+ * applied electric field and time" is BC = 0 in those two directions (set by orc_set_boundary).             */
+static double BC[4] = {1.0, 1.0, 1.0, -1.0};
+
+void orc_set_boundary(const double *bc4)
+{
+    for (int mu = 0; mu < 4; mu++) BC[mu] = bc4[mu];
+}
+
 /* neighbour of site (c[0..3]) one step in direction mu (dir=+1/-1), periodic index; *phase gets the
- * boundary factor: -1 when the hop crosses between t=T-1 and t=0, +1 otherwise
- * (north_star: periodic in space, antiperiodic in time; reading G11).                     */
+ * boundary factor BC[mu] when the hop crosses between coordinate d[mu]-1 and 0, +1 otherwise.             */
 static long neighbour(const int *d, const int *c, int mu, int dir, double *phase)
 {
     int n[4] = {c[0], c[1], c[2], c[3]};
@@ -60,11 +70,11 @@ static long neighbour(const int *d, const int *c, int mu, int dir, double *phase
     *phase = 1.0;
     if (n[mu] >= d[mu]) {
         n[mu] -= d[mu];
-        if (mu == 3) *phase = -1.0;
+        *phase = BC[mu];
     }
     if (n[mu] < 0) {
         n[mu] += d[mu];
-        if (mu == 3) *phase = -1.0;
+        *phase = BC[mu];
     }
     return n[0] + (long)d[0] * (n[1] + (long)d[1] * (n[2] + (long)d[2] * n[3]));
 }

@@ -91,6 +91,13 @@ def host_eigh(A: np.ndarray):
     return w, Z
 
 
+class OvOptions(ctypes.Structure):
+    """struct ov_options of include/ov.h."""
+    _fields_ = [("layout", ctypes.c_int), ("t_boundary", ctypes.c_int), ("wall_mask", ctypes.c_int),
+                ("field", ctypes.c_int), ("field_origin", ctypes.c_int), ("reserved", ctypes.c_int),
+                ("field_qE", ctypes.c_double)]
+
+
 class Overlap:
     """One ov_ctx.  Spinor arguments are torch complex128 CUDA tensors in the ABI layout [nrhs?][12][V]
     unless a method says "canonical" ([T][Z][Y][X][4][3])."""
@@ -98,7 +105,10 @@ class Overlap:
     LAYOUTS = {"auto": 0, "blocked": 1, "planes": 2}
     BOUNDARIES = {"antiperiodic": 0, "periodic": 1, "open": 2}
 
-    def __init__(self, dims, kappa, gauge, recon=18, stream=None, layout="auto", t_boundary="antiperiodic"):
+    def __init__(self, dims, kappa, gauge, recon=18, stream=None, layout="auto", t_boundary="antiperiodic",
+                 walls=(), field_dir=None, field_qE=0.0, field_origin=0):
+        """walls: space directions (0, 1, 2) with a Dirichlet wall; field_dir: direction of a constant electric
+        field of strength field_qE (None = no field).  See ov_options in include/ov.h."""
         if not torch.cuda.is_available():
             raise OvError(OV_ECUDA, "no CUDA device: this library has no CPU fallback")
         self.lib = load_library()
@@ -111,9 +121,10 @@ class Overlap:
         self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         self._ctx = ctypes.c_void_p()
         cdims = (ctypes.c_int * 4)(*self.dims)
-        opt = (ctypes.c_int * 8)(self.LAYOUTS[layout], self.BOUNDARIES[t_boundary], 0, 0, 0, 0, 0, 0)   # struct ov_options
+        opt = OvOptions(self.LAYOUTS[layout], self.BOUNDARIES[t_boundary], sum(1 << int(mu) for mu in walls),
+                        0 if field_dir is None else int(field_dir) + 1, int(field_origin), 0, float(field_qE))
         rc = self.lib.ov_create_ex(ctypes.byref(self._ctx), cdims, ctypes.c_double(kappa), _ptr(gauge.contiguous()),
-                                   ctypes.c_int(recon), ctypes.c_void_p(self.stream.cuda_stream), opt)
+                                   ctypes.c_int(recon), ctypes.c_void_p(self.stream.cuda_stream), ctypes.byref(opt))
         if rc != OV_OK:
             raise OvError(rc, "ov_create failed")
         self._keepalive = None

@@ -126,8 +126,8 @@ int ov_create_ex(ov_ctx** out, const int dims[4], double kappa, const void* gaug
     ov_options opt{};
     if (options) opt = *options;
     if (opt.layout < 0 || opt.layout > 2 || opt.t_boundary < 0 || opt.t_boundary > 2) return OV_EINVAL;
-    for (int r : opt.reserved)
-        if (r != 0) return OV_EINVAL;
+    if (opt.reserved != 0 || opt.wall_mask < 0 || opt.wall_mask > 7 || opt.field < 0 || opt.field > 3) return OV_EINVAL;
+    if (opt.field != 0 && (recon != 18 || !std::isfinite(opt.field_qE))) return OV_EINVAL;   // U(3) links need all 18 reals
     *out = nullptr;
     if (!dims || !gauge_dev) return OV_EINVAL;
     if (recon != 18 && recon != 12) return OV_EINVAL;
@@ -154,7 +154,12 @@ int ov_create_ex(ov_ctx** out, const int dims[4], double kappa, const void* gaug
         rc = gauge_su3_defect(ctx, (const double2*)gauge_dev, &defect);
         if (rc == OV_OK && !(defect <= 1e-9)) rc = OV_EINVAL;
     }
-    if (rc == OV_OK) rc = launch_gauge_relayout(ctx, (const double2*)gauge_dev);
+    GaugeMods mods{};
+    mods.wall_mask = opt.wall_mask;
+    mods.field_dir = opt.field - 1;
+    mods.qE = opt.field_qE;
+    mods.origin = opt.field_origin;
+    if (rc == OV_OK) rc = launch_gauge_relayout(ctx, (const double2*)gauge_dev, &mods);
     if (rc == OV_OK && cudaStreamSynchronize(ctx->stream) != cudaSuccess) rc = OV_ECUDA;
     if (rc == OV_OK) rc = ensure_reduction_buffers(ctx, 1, 1024);
     if (rc != OV_OK) { ov_destroy(ctx); return rc; }

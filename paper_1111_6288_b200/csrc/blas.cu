@@ -12,15 +12,39 @@
 namespace ov {
 
 // ------------------------------------------------------------------------------------------ layout
-// canonical gauge [site][mu][9] -> internal layout (gauge_index, ov_internal.h)
-template <int NE, bool BL>
-__global__ void gauge_relayout_kernel(const double2* __restrict__ can, double2* __restrict__ g, long long V) {
+// canonical gauge [site][mu][9] -> internal layout (gauge_index, ov_internal.h).  MOD: the links are modified on the way
+// (ov_options): U_t(x) *= exp(-i qE (x_dir - origin)) (eq. 4.1 with A_t = E (x_dir - origin)) and the
+// links across a Dirichlet wall (coordinate d_mu - 1 in a direction of wall_mask) are set to zero.
+template <int NE, bool BL, bool MOD>
+__global__ void gauge_relayout_kernel(const double2* __restrict__ can, double2* __restrict__ g, long long V, GaugeMods m) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= V) return;
+    int c[4];
+    double2 ph = make_double2(1.0, 0.0);
+    if (MOD) {
+        long long r = i;
+        c[0] = (int)(r % m.X); r /= m.X;
+        c[1] = (int)(r % m.Y); r /= m.Y;
+        c[2] = (int)(r % m.Z); r /= m.Z;
+        c[3] = (int)r;
+        if (m.field_dir >= 0) {
+            double sn, cs;
+            sincos(-m.qE * (double)(c[m.field_dir] - m.origin), &sn, &cs);
+            ph = make_double2(cs, sn);
+        }
+    }
+    const int ext[4] = {m.X, m.Y, m.Z, m.T};
 #pragma unroll
-    for (int mu = 0; mu < 4; mu++)
+    for (int mu = 0; mu < 4; mu++) {
+        const bool wall = MOD && ((m.wall_mask >> mu) & 1) && c[mu] == ext[mu] - 1;
 #pragma unroll
-        for (int e = 0; e < NE; e++) g[gauge_index<NE, BL>(V, mu, e, i)] = can[(i * 4 + mu) * 9 + e];
+        for (int e = 0; e < NE; e++) {
+            double2 u = can[(i * 4 + mu) * 9 + e];
+            if (MOD && mu == 3 && m.field_dir >= 0) u = make_double2(u.x * ph.x - u.y * ph.y, u.x * ph.y + u.y * ph.x);
+            if (wall) u = make_double2(0.0, 0.0);
+            g[gauge_index<NE, BL>(V, mu, e, i)] = u;
+        }
+    }
 }
 
 // largest |row2 - conj(row0 x row1)| and |<row_i,row_j> - delta_ij| over all links: recon 12 is only valid for SU(3)
@@ -69,17 +93,26 @@ int gauge_su3_defect(ov_ctx* ctx, const double2* canonical, double* defect) {
     return OV_OK;
 }
 
-int launch_gauge_relayout(ov_ctx* ctx, const double2* canonical) {
+int launch_gauge_relayout(ov_ctx* ctx, const double2* canonical, const GaugeMods* mods) {
     const long long V = ctx->lat.V;
     const int threads = 128;
     const unsigned blocks = (unsigned)((V + threads - 1) / threads);
+    GaugeMods m{};
+    m.field_dir = -1;
+    const bool mod = mods && (mods->wall_mask || mods->field_dir >= 0);
+    if (mod) m = *mods;
+    m.X = ctx->lat.X; m.Y = ctx->lat.Y; m.Z = ctx->lat.Z; m.T = ctx->lat.T;
+#define OV_RELAYOUT(NE, BL)                                                                                          \
+    do {                                                                                                             \
+        if (mod) gauge_relayout_kernel<NE, BL, true><<<blocks, threads, 0, ctx->stream>>>(canonical, ctx->gauge, V, m); \
+        else gauge_relayout_kernel<NE, BL, false><<<blocks, threads, 0, ctx->stream>>>(canonical, ctx->gauge, V, m);   \
+    } while (0)
     if (ctx->recon == 12) {
-        if (ctx->blocked) gauge_relayout_kernel<6, true><<<blocks, threads, 0, ctx->stream>>>(canonical, ctx->gauge, V);
-        else gauge_relayout_kernel<6, false><<<blocks, threads, 0, ctx->stream>>>(canonical, ctx->gauge, V);
+        if (ctx->blocked) OV_RELAYOUT(6, true); else OV_RELAYOUT(6, false);
     } else {
-        if (ctx->blocked) gauge_relayout_kernel<9, true><<<blocks, threads, 0, ctx->stream>>>(canonical, ctx->gauge, V);
-        else gauge_relayout_kernel<9, false><<<blocks, threads, 0, ctx->stream>>>(canonical, ctx->gauge, V);
+        if (ctx->blocked) OV_RELAYOUT(9, true); else OV_RELAYOUT(9, false);
     }
+#undef OV_RELAYOUT
     ctx->launches++;
     OV_CUDA(ctx, cudaGetLastError());
     return OV_OK;

@@ -135,7 +135,15 @@ int workspace(ov_ctx* ctx, int i, double2** out);
 int ensure_reduction_buffers(ov_ctx* ctx, size_t partial_elems, size_t result_elems);
 
 // --- kernels (launchers); all enqueue on ctx->stream and bump ctx->launches ---
-int launch_gauge_relayout(ov_ctx* ctx, const double2* canonical);
+// link modifications applied while the gauge field is re-laid out (ov_options: background field, Dirichlet walls)
+struct GaugeMods {
+    int X, Y, Z, T;
+    int wall_mask;   // bit mu: links across the boundary in direction mu are zero
+    int field_dir;   // -1 none; 0..2: U_t(x) *= exp(-i qE (x_dir - origin))
+    double qE;
+    int origin;
+};
+int launch_gauge_relayout(ov_ctx* ctx, const double2* canonical, const GaugeMods* mods = nullptr);
 int gauge_su3_defect(ov_ctx* ctx, const double2* canonical, double* defect);
 int launch_pack(ov_ctx* ctx, const double2* canonical, double2* abi);
 int launch_unpack(ov_ctx* ctx, const double2* abi, double2* canonical);

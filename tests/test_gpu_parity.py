@@ -390,7 +390,9 @@ def test_tma_variant_sign_and_dov_vs_oracle(ovp, recon):
         s, d = to_host(op, op.apply_sign(dx)), to_host(op, op.apply_dov(0.07, dx))
         assert rel(s, ref_s) <= TOL_DOV and rel(d, ref_d) <= TOL_DOV
         out[variant] = (s, d)
-    assert np.array_equal(out[1][0], out[2][0]) and np.array_equal(out[1][1], out[2][1])
+    # same arithmetic in the same order; the compiler's FMA contraction may differ between the two kernels
+    print(f"  TMA-staged vs gather kernel, recon {recon}: sign {rel(out[1][0], out[2][0]):.3e}, D_ov {rel(out[1][1], out[2][1]):.3e}")
+    assert rel(out[1][0], out[2][0]) <= 1e-14 and rel(out[1][1], out[2][1]) <= 1e-14
 
 
 # ------------------------------------------------------------------------------------------ links that are not SU(3)
@@ -410,6 +412,39 @@ def test_u3_and_dirichlet_links(ovp):
     with pytest.raises(ovp.OvError):
         make(ovp, dims, Ub, recon=12)
     make(ovp, dims, U, recon=12)                                           # genuine SU(3) links are accepted
+
+
+@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("t_boundary,bc_t", [("periodic", 1.0), ("open", 0.0), ("antiperiodic", -1.0)])
+def test_background_field_and_boundaries_api_vs_oracle(ovp, variant, t_boundary, bc_t):
+    """The library's own background field + Dirichlet walls (ov_options: field, wall_mask, t_boundary)
+    against the oracle fed with the links of workloads.background_field / the oracle's boundary factors: the two sides
+    implement eq. 4.1 and the walls independently.  8^3 x 16 (configs[1] shape), both Wilson kernels, H_w and D_ov."""
+    dims = (8, 8, 8, 16)
+    qE, fdir, org = 0.0123, 1, 3
+    U = wl.su3_links(dims, 0.5, 61)
+    x = wl.gaussian_source(dims, 62)
+    Uo = wl.background_field(U, dims, qE, fdir, origin=org)              # oracle side: the field as input links
+    bc = (1.0, 0.0, 1.0, bc_t)                                           # wall in y (the field direction), t as asked
+    op = ovp.Overlap(dims, KAPPA, U, recon=18, t_boundary=t_boundary, walls=(fdir,), field_dir=fdir, field_qE=qE,
+                     field_origin=org)
+    op.set_dslash_variant(variant)
+    se, n = 0.2, 10
+    coef = ovp.chebyshev_coeffs(n, se * se)
+    op.set_polynomial(coef, se * se, NORM)
+    dx = to_dev(op, x)
+    with oracle.boundary(bc):
+        ref_h = oracle.hw(dims, KAPPA, Uo, x)
+        ref_d = oracle.dov(dims, KAPPA, Uo, coef, se * se, NORM, None, None, 0.05, x)
+    assert rel(to_host(op, op.apply_hw(dx)), ref_h) <= TOL_HW
+    assert rel(to_host(op, op.apply_dov(0.05, dx)), ref_d) <= TOL_DOV
+    assert rel(ref_h, oracle.hw(dims, KAPPA, U, x)) > 1e-3               # the field and the walls do matter
+    with pytest.raises(ovp.OvError):                                     # U(3) links cannot be rebuilt from 12 reals
+        ovp.Overlap(dims, KAPPA, U, recon=12, field_dir=fdir, field_qE=qE)
+    op12 = ovp.Overlap(dims, KAPPA, U, recon=12, t_boundary=t_boundary, walls=(fdir,))   # walls alone: fine with recon 12
+    with oracle.boundary(bc):
+        ref12 = oracle.hw(dims, KAPPA, U, x)
+    assert rel(to_host(op12, op12.apply_hw(to_dev(op12, x))), ref12) <= TOL_HW
 
 
 # ------------------------------------------------------------------------------------------ degenerate cases

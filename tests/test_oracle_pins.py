@@ -369,3 +369,72 @@ def test_golden_lowmodes_file_is_this_operator():
     assert th[0] >= gold[0] ** 2 * (1 - 1e-9)             # variational: no Ritz value below the lowest eigenvalue
     assert th[0] <= gold[-1] ** 2                          # ... and the Krylov space has reached the stored cluster
     assert th[-1] <= 1.0                                   # norm = 1 + 8 kappa bounds the spectrum of Q
+
+
+# ---------------------------------------------------------------- boundary modes and background field
+def test_P13_periodic_time_plane_wave():
+    """With the t boundary set periodic the free plane waves carry p_t = 2 pi n / T (not (2n+1) pi / T): pins that the
+    boundary factor sits on the hop across t = T-1 <-> 0 and nowhere else."""
+    dims = (4, 2, 6, 8)
+    U = wl.unit_links(dims)
+    rng = np.random.default_rng(6)
+    p = (2 * np.pi * 1 / 4, 2 * np.pi * 1 / 2, 2 * np.pi * 5 / 6, 2 * np.pi * 3 / 8)
+    u = rng.standard_normal(12) + 1j * rng.standard_normal(12)
+    psi = _plane_wave(dims, p, u)
+    M = (1.0 - 2.0 * KAPPA * sum(np.cos(p))) * np.eye(4, dtype=complex)
+    for mu in range(4):
+        M = M + 2j * KAPPA * np.sin(p[mu]) * oracle.gamma(mu)
+    expect = g5(_plane_wave(dims, p, (M @ u.reshape(4, 3)).reshape(12)))
+    with oracle.boundary((1, 1, 1, 1)):
+        got = oracle.hw(dims, KAPPA, U, psi)
+    assert rel(got, expect) < 1e-13
+    assert rel(oracle.hw(dims, KAPPA, U, psi), expect) > 1e-2      # the default (antiperiodic) is back and differs
+
+
+def test_P14_dirichlet_equals_zero_links_and_is_hermitian():
+    """Boundary factor 0 in a direction = periodic operator on links whose wall links are zero (two routes to the same
+    operator: the factor in neighbour() vs the generator's zeroed links), and H_w stays Hermitian."""
+    dims = (4, 2, 6, 4)
+    U = wl.su3_links(dims, 0.6, 21)
+    psi = wl.gaussian_source(dims, 22)
+    phi = wl.gaussian_source(dims, 23)
+    for dirs in [(3,), (1, 3), (0, 2)]:
+        bc = [1.0, 1.0, 1.0, -1.0]
+        for mu in dirs:
+            bc[mu] = 0.0
+        with oracle.boundary(bc):
+            a = oracle.hw(dims, KAPPA, U, psi)
+            lhs = vdot(phi, a)
+            rhs = vdot(oracle.hw(dims, KAPPA, U, phi), psi)
+        b = oracle.hw(dims, KAPPA, wl.dirichlet_walls(U, dims, dirs), psi)
+        assert rel(a, b) < 1e-15
+        assert abs(lhs - rhs) / abs(lhs) < 1e-13
+        assert rel(a, oracle.hw(dims, KAPPA, U, psi)) > 1e-3
+
+
+def test_P15_background_field_plaquette_and_gauge_equivalence():
+    """Generator pins (eq. 4.1): every (direction, t) plaquette of the field on unit links is exp(-i qE); and with
+    Dirichlet walls in `direction` and t the spectrum cannot depend on `origin` (a constant shift of A_t is a pure
+    gauge exp(-i qE origin t)): H_w[origin = 2] = g H_w[origin = 0] g^+ with g(t) = exp(i qE origin t)... checked on a vector."""
+    dims = (4, 6, 2, 8)
+    X, Y, Z, T = dims
+    qE, d = 0.37, 1
+    B = wl.background_field(wl.unit_links(dims), dims, qE, d)
+    Ud, Ut = B[..., d, 0, 0], B[..., 3, 0, 0]                       # [T][Z][Y][X] phases
+    ax = 3 - d
+    plaq = Ud * np.roll(Ut, -1, axis=ax) * np.conj(np.roll(Ud, -1, axis=0)) * np.conj(Ut)
+    interior = [slice(0, T - 1), slice(None), slice(None), slice(None)]
+    interior[ax] = slice(0, dims[d] - 1)
+    assert np.max(np.abs(plaq[tuple(interior)] - np.exp(-1j * qE))) < 1e-14
+    # origin independence under Dirichlet walls
+    U = wl.su3_links(dims, 0.5, 31)
+    psi = wl.gaussian_source(dims, 32)
+    org = 2
+    U0 = wl.dirichlet_walls(wl.background_field(U, dims, qE, d, origin=0), dims, (d, 3))
+    U2 = wl.dirichlet_walls(wl.background_field(U, dims, qE, d, origin=org), dims, (d, 3))
+    t = np.arange(T).reshape(T, 1, 1, 1, 1, 1)
+    g = np.exp(-1j * qE * org * t)                                   # psi'(t) = g(t) psi(t)
+    with oracle.boundary((1, 0, 1, 0)):
+        lhs = oracle.hw(dims, KAPPA, U2, g * psi)
+        rhs = g * oracle.hw(dims, KAPPA, U0, psi)
+    assert rel(lhs, rhs) < 1e-13

@@ -15,6 +15,8 @@ from .generators import (  # noqa: F401
     su3_links,
     unit_links,
     su3_field,
+    background_field,
+    dirichlet_walls,
     gaussian_source,
     point_source,
     gauge_seed,

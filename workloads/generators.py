@@ -69,6 +69,35 @@ def unit_links(dims) -> np.ndarray:
     return U
 
 
+def background_field(U: np.ndarray, dims, qE: float, direction: int, origin: int = 0) -> np.ndarray:
+    """Constant electric field of strength E along `direction` (0, 1, 2 = x, y, z) for a quark of charge q, as input
+    links (eq. 4.1: U_mu -> exp(-i q A_mu) U_mu).  Gauge taken here (the paper does not fix it):
+    A_t(x) = E (x_direction - origin), all other components zero, i.e. only the t links get the phase
+    exp(-i qE (x_direction - origin)); every (direction, t) plaquette then carries exp(-i qE).  Returns a new array;
+    the links are U(3), not SU(3).  Meant to be used with Dirichlet walls in `direction` and t (dirichlet_walls)."""
+    X, Y, Z, T = (int(d) for d in dims)
+    if direction not in (0, 1, 2):
+        raise ValueError("direction must be 0, 1 or 2")
+    out = np.array(U, dtype=np.complex128, copy=True)
+    coord = np.arange((X, Y, Z)[direction], dtype=np.float64) - float(origin)
+    shape = [1, 1, 1, 1]                     # [T][Z][Y][X]
+    shape[3 - direction] = coord.size
+    phase = np.exp(-1j * float(qE) * coord).reshape(shape)
+    out[..., 3, :, :] *= phase[..., None, None]
+    return out
+
+
+def dirichlet_walls(U: np.ndarray, dims, directions) -> np.ndarray:
+    """Links with Dirichlet walls: the links that cross the lattice boundary in each of `directions`
+    (U_mu at coordinate d_mu - 1) are set to zero, so no hop connects coordinate d_mu - 1 and 0."""
+    out = np.array(U, dtype=np.complex128, copy=True)
+    for mu in directions:
+        idx = [slice(None)] * 4              # [T][Z][Y][X]
+        idx[3 - int(mu)] = -1
+        out[tuple(idx) + (int(mu),)] = 0.0
+    return out
+
+
 def gaussian_source(dims, seed: int) -> np.ndarray:
     """Gaussian random spinor, complex128 [T][Z][Y][X][4][3], re then im drawn N(0,1)."""
     X, Y, Z, T = (int(d) for d in dims)
