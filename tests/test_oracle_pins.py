@@ -438,3 +438,76 @@ def test_P15_background_field_plaquette_and_gauge_equivalence():
         lhs = oracle.hw(dims, KAPPA, U2, g * psi)
         rhs = g * oracle.hw(dims, KAPPA, U0, psi)
     assert rel(lhs, rhs) < 1e-13
+
+
+# ---------------------------------------------------------------- low modes of D_ov and deflation
+from oracle import deflation as dfl  # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def hard4():
+    """4^4, smooth links, PERIODIC time: D_ov has 12 near-zero modes (the lifted p = 0 modes of the free field)."""
+    dims = (4, 4, 4, 4)
+    U = wl.su3_links(dims, 0.3, 41)
+    bc = (1.0, 1.0, 1.0, 1.0)
+    with oracle.boundary(bc):
+        w, Zv, H, herm = dense.eig_hw(dims, KAPPA, U)
+    assert herm < 1e-13
+    A = dfl.dense_normal(w, Zv)
+    return dict(dims=dims, U=U, bc=bc, w=w, Zv=Zv, A=A, shape=(4, 4, 4, 4, 4, 3))
+
+
+def test_P16_normal_operator_chirality_structure(hard4):
+    """With the exact sign: A = gamma5 D gamma5 D commutes with gamma5; on a chiral vector it equals the one-sign form
+    2x + (s + gamma5) S x; its spectrum lies in [0, 4]; the non-zero levels of the two sectors coincide (pairing)."""
+    c = hard4
+    A, shape = c["A"], c["shape"]
+    N = A.shape[0]
+    g5 = np.tile(np.repeat([1.0, 1.0, -1.0, -1.0], 3), N // 12)
+    assert np.max(np.abs(A * g5[None, :] - g5[:, None] * A)) < 1e-12             # [A, gamma5] = 0
+    assert np.max(np.abs(A - A.conj().T)) < 1e-12
+    S = dfl.dense_sign(c["w"], c["Zv"])
+    x = wl.gaussian_source(c["dims"], 42)
+
+    def dov0(v):                                                                  # D_ov(0) v with the exact sign
+        return v + dfl.gamma5((S @ v.reshape(-1)).reshape(shape))
+
+    ref = dfl.normal_op(dov0, x)
+    assert rel((A @ x.reshape(-1)).reshape(shape), ref) < 1e-12
+    for s in (+1, -1):
+        xs = dfl.chiral_project(x, s)
+        one_sign = dfl.sector_op(lambda v: (S @ v.reshape(-1)).reshape(shape), s, xs)
+        assert rel(one_sign, dfl.normal_op(dov0, xs)) < 1e-12
+        assert rel(dfl.gamma5(one_sign), s * one_sign) < 1e-12                    # stays in its sector
+    mu_p, _ = dfl.dense_sector_modes(A, +1, N // 2, shape)
+    mu_m, _ = dfl.dense_sector_modes(A, -1, N // 2, shape)
+    assert mu_p.min() > -1e-12 and mu_p.max() < 4 + 1e-12 and mu_m.min() > -1e-12 and mu_m.max() < 4 + 1e-12
+    inner_p = mu_p[(mu_p > 1e-9) & (mu_p < 4 - 1e-9)]
+    inner_m = mu_m[(mu_m > 1e-9) & (mu_m < 4 - 1e-9)]
+    assert len(inner_p) == len(inner_m) and np.max(np.abs(inner_p - inner_m)) < 1e-10
+    assert mu_p[5] < 0.02 and mu_p[6] > 0.3                                       # 6 near-zero modes per sector, then a gap
+
+
+def test_P17_deflated_multishift_cg_vs_direct_solve(hard4):
+    """Deflated multi-mass CG = dense direct solve for every shift; deflating the 6 + 6 near-zero modes cuts the
+    iteration count by more than 3 (PAPER.md:45 quotes 3-4 at m_pi ~ 200 MeV)."""
+    c = hard4
+    A, shape = c["A"], c["shape"]
+    N = A.shape[0]
+    b = wl.gaussian_source(c["dims"], 43)
+    sig = [sigma_of_mass(m) for m in (0.005, 0.02, 0.1)]
+
+    def apply_A(v):
+        return (A @ v.reshape(-1)).reshape(shape)
+
+    mu_p, W_p = dfl.dense_sector_modes(A, +1, 6, shape)
+    mu_m, W_m = dfl.dense_sector_modes(A, -1, 6, shape)
+    W = np.concatenate([W_p, W_m])
+    mu = np.concatenate([mu_p, mu_m])
+    xs, it_defl, res = dfl.deflated_multishift_cg(apply_A, W, mu, sig, b, 1e-9, 2000)
+    _, it_plain, res_plain = multishift_cg(apply_A, sig, b, 1e-9, 2000)
+    assert np.all(res <= 1e-8) and np.all(res_plain <= 1e-8)
+    for s, x in zip(sig, xs):
+        direct = np.linalg.solve(A + s * np.eye(N), b.reshape(-1)).reshape(shape)
+        assert rel(x, direct) < 1e-6
+    assert it_plain >= 3 * it_defl, (it_plain, it_defl)
