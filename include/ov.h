@@ -205,6 +205,29 @@ int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_restarts, int ch
  * lambda^2 < a are amplified), times the window had to be widened (completeness guard), Krylov dimension m }.  */
 int ov_lanczos_stats(const ov_ctx* ctx, double* out_host);
 
+/* ---- low modes of the overlap operator and deflation ("we use deflation to help speed up
+ * the calculation.  This consists of computing the low lying spectrum of the overlap operator", :81 "Chebyshev order of
+ * 12 ... the 100 lowest eigenmodes for the overlap operator"; reading G20) ------------------------------
+ * ov_lanczos_dov_lowmodes: the k lowest eigenpairs (mu_i, w_i) of A = D_ov(0)^+ D_ov(0) in ONE chirality sector
+ *   (chirality = +1 or -1, gamma5 w_i = chirality w_i), where A acts as  A_s x = 2 x + (s + gamma5) sign(H_w) x  (one
+ *   sign per application; = gamma5 D_ov gamma5 D_ov up to 1 - sign^2 = O(delta)).  A commutes with gamma5 and every
+ *   level 0 < mu < 4 occurs once in each sector, so the low modes of A are the union of the two sectors' runs.  Needs
+ *   ov_set_polynomial (and ov_set_smallspace where the polynomial needs it).  Same driver, arguments, memory behaviour
+ *   and return codes as ov_lanczos_lowmodes; cheb_order = degree of the filter in A_s (paper: 12), each filter term
+ *   costs one sign(H_w).  W_out_dev: k ABI spinors; mu_out_host ascending; resid_i = |A_s w_i - mu_i w_i| <= tol.
+ * ov_set_deflation: hands k orthonormal eigenpairs of A to ov_multishift_cg (W_dev is BORROWED until replaced or
+ *   ov_set_deflation(ctx, NULL, NULL, 0); mu_host is copied).  The solver then returns
+ *       x_i = sum_j w_j (w_j^+ b)/(mu_j + sigma_i) + [multi-shift CG on b - W W^+ b],
+ *   still stopping at |r| <= tol |b| and reporting true residuals of the full systems.  PRECONDITION: the w_j are
+ *   eigenvectors of the operator the CG applies (gamma5 D_ov gamma5 D_ov with the current polynomial) to within tol,
+ *   i.e. eigensolver residual and polynomial error delta (the sector form differs from gamma5 D gamma5 D by
+ *   1 - sign^2 = O(delta)) both <~ tol (mu_j + sigma_i): the defect of w_j enters x_i amplified by 1/(mu_j + sigma_i);
+ *   otherwise the true residuals stall near max(delta, resid) |W^+ b| / min(mu + sigma) and relres_out shows it.  Do not combine with ov_set_cg_adaptive
+ *   modes 1-2 (an inexact A re-populates the deflated directions).                                                 */
+int ov_lanczos_dov_lowmodes(ov_ctx* ctx, int chirality, int k, double tol, int max_restarts, int cheb_order,
+                            int subspace, void* W_out_dev, double* mu_out_host, double* resid_out_host);
+int ov_set_deflation(ov_ctx* ctx, const void* W_dev, const double* mu_host, int k);
+
 /* ---- host-logic test hook (no device work): eigen-decomposition of a dense n x n Hermitian matrix by the
  * cyclic complex Jacobi routine the Lanczos driver uses.  A_host: row-major (re,im) pairs; w_out: n ascending
  * eigenvalues; Z_out: row-major (re,im), eigenvectors as columns.                                            */

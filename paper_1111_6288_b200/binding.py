@@ -25,7 +25,7 @@ SYMBOLS = [
     "ov_set_dslash_variant", "ov_get_dslash_variant", "ov_pack_spinor", "ov_unpack_spinor", "ov_dslash", "ov_apply_hw",
     "ov_chebyshev_coeffs", "ov_set_polynomial", "ov_set_smallspace", "ov_project", "ov_apply_sign",
     "ov_apply_dov", "ov_apply_dov_reduced", "ov_apply_hw_f32", "ov_set_cg_adaptive", "ov_cg_orders", "ov_apply_hw_host", "ov_apply_dov_host", "ov_blas_axpy", "ov_blas_scale", "ov_blas_dot",
-    "ov_blas_norm2", "ov_multishift_cg", "ov_lanczos_lowmodes", "ov_lanczos_stats", "ov_host_eigh",
+    "ov_blas_norm2", "ov_multishift_cg", "ov_lanczos_lowmodes", "ov_lanczos_stats", "ov_lanczos_dov_lowmodes", "ov_set_deflation", "ov_host_eigh",
 ]
 
 
@@ -315,6 +315,30 @@ class Overlap:
         if rc not in (OV_OK, OV_ENOCONV):
             self._check(rc)
         return V, lam, res, rc == OV_OK
+
+    def lanczos_dov_lowmodes(self, chirality, k, tol=1e-9, max_restarts=50, cheb_order=12, subspace=0):
+        """ov_lanczos_dov_lowmodes: k lowest eigenpairs of D_ov^+ D_ov in one chirality sector (+1 / -1)."""
+        W = self.new_spinor(k)
+        mu, res = np.empty(k), np.empty(k)
+        rc = self.lib.ov_lanczos_dov_lowmodes(self._ctx, ctypes.c_int(chirality), ctypes.c_int(k), ctypes.c_double(tol),
+                                              ctypes.c_int(max_restarts), ctypes.c_int(cheb_order), ctypes.c_int(subspace),
+                                              _ptr(W), mu.ctypes.data_as(ctypes.POINTER(ctypes.c_double)),
+                                              res.ctypes.data_as(ctypes.POINTER(ctypes.c_double)))
+        if rc not in (OV_OK, OV_ENOCONV):
+            self._check(rc)
+        return W, mu, res, rc == OV_OK
+
+    def set_deflation(self, W, mu):
+        """ov_set_deflation: W [k][12][V] eigenvectors of D_ov^+ D_ov (kept alive here), mu their eigenvalues; None clears."""
+        if W is None:
+            self._check(self.lib.ov_set_deflation(self._ctx, None, None, ctypes.c_int(0)))
+            self._defl = None
+            return
+        mu = np.ascontiguousarray(mu, dtype=np.float64)
+        assert W.is_cuda and W.dtype == torch.complex128 and W.is_contiguous() and W.shape[0] == len(mu)
+        self._check(self.lib.ov_set_deflation(self._ctx, _ptr(W), mu.ctypes.data_as(ctypes.POINTER(ctypes.c_double)),
+                                              ctypes.c_int(len(mu))))
+        self._defl = W
 
     def lanczos_stats(self):
         """ov_lanczos_stats: counters of the last lanczos_lowmodes call."""

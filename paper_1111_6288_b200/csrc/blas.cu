@@ -213,6 +213,40 @@ __global__ void __launch_bounds__(kEwThreads) gamma5_kernel(const double2* x, do
     }
 }
 
+// z = a x + b y + c w (real a, b, c); z may alias any operand (the generic Chebyshev filter of the D_ov eigensolver)
+__global__ void __launch_bounds__(kEwThreads) axpbypcz_kernel(double a, const double2* x, double b, const double2* y,
+                                                              double c, const double2* w, double2* z, long long n) {
+    const long long base = (long long)blockIdx.x * (kEwThreads * kEw) + threadIdx.x;
+#pragma unroll
+    for (int m = 0; m < kEw; m++) {
+        const long long e = base + (long long)m * kEwThreads;
+        if (e < n) {
+            const double2 xv = x[e], yv = y[e], wv = w[e];
+            z[e] = make_double2(fma(c, wv.x, fma(b, yv.x, a * xv.x)), fma(c, wv.y, fma(b, yv.y, a * xv.y)));
+        }
+    }
+}
+
+// out = ax x + (s + gamma5) y : the chirality-sector form of D_ov^+ D_ov (ax = 2, y = sign(H_w) x), or the
+// projector 2 P_s y with ax = 0 (x may then be null).  Upper components (spins 0,1) get (s + 1) y, lower ones (s - 1) y.
+__global__ void __launch_bounds__(kEwThreads) chiral_combine_kernel(double ax, const double2* x, double s, const double2* y,
+                                                                    double2* out, long long V, int blocked) {
+    const long long n = 12 * V;
+    const long long base = (long long)blockIdx.x * (kEwThreads * kEw) + threadIdx.x;
+#pragma unroll
+    for (int m = 0; m < kEw; m++) {
+        const long long e = base + (long long)m * kEwThreads;
+        if (e < n) {
+            const bool lower = blocked ? ((e >> 5) % 12) >= 6 : e >= 6 * V;
+            const double f = lower ? s - 1.0 : s + 1.0;
+            const double2 yv = y[e];
+            double2 v = make_double2(f * yv.x, f * yv.y);
+            if (x) { const double2 xv = x[e]; v.x = fma(ax, xv.x, v.x); v.y = fma(ax, xv.y, v.y); }
+            out[e] = v;
+        }
+    }
+}
+
 static inline unsigned ew_blocks(long long n) { return (unsigned)((n + kEwThreads * kEw - 1) / (kEwThreads * kEw)); }
 
 int launch_axpy(ov_ctx* ctx, double2 a, const double2* x, double2* y) {
@@ -225,6 +259,20 @@ int launch_axpy(ov_ctx* ctx, double2 a, const double2* x, double2* y) {
 int launch_axpby(ov_ctx* ctx, double a, const double2* x, double b, const double2* y, double2* z, int nrhs) {
     const long long n = (long long)spinor_elems(ctx) * nrhs;
     axpby_kernel<<<ew_blocks(n), kEwThreads, 0, ctx->stream>>>(a, x, b, y, z, n);
+    ctx->launches++;
+    OV_CUDA(ctx, cudaGetLastError());
+    return OV_OK;
+}
+int launch_axpbypcz(ov_ctx* ctx, double a, const double2* x, double b, const double2* y, double c, const double2* w, double2* z) {
+    const long long n = (long long)spinor_elems(ctx);
+    axpbypcz_kernel<<<ew_blocks(n), kEwThreads, 0, ctx->stream>>>(a, x, b, y, c, w, z, n);
+    ctx->launches++;
+    OV_CUDA(ctx, cudaGetLastError());
+    return OV_OK;
+}
+int launch_chiral_combine(ov_ctx* ctx, double ax, const double2* x, int s, const double2* y, double2* out) {
+    const long long n = (long long)spinor_elems(ctx);
+    chiral_combine_kernel<<<ew_blocks(n), kEwThreads, 0, ctx->stream>>>(ax, x, (double)s, y, out, ctx->lat.V, ctx->blocked ? 1 : 0);
     ctx->launches++;
     OV_CUDA(ctx, cudaGetLastError());
     return OV_OK;

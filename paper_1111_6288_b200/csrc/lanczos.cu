@@ -13,6 +13,7 @@
 // copy of the basis (the paper's 2.5 l subspace, would be 201 GB there).
 #include <algorithm>
 #include <cmath>
+#include <functional>
 #include <numeric>
 
 #include "ov_internal.h"
@@ -55,6 +56,37 @@ static int apply_filter(ov_ctx* ctx, const Filter& f, const double2* in, double2
         e3.A1 = cur; e3.a1 = -2.0 * cs;
         e3.A2 = prev; e3.a2 = -1.0;
         OV_TRY(launch_wilson(ctx, tq, buf(j), e3));
+    }
+    return OV_OK;
+}
+
+// The eigenproblem the driver below works on: the wanted modes are the LOWEST eigenvalues of a Hermitian positive
+// semi-definite "base" operator B with spectrum in [0, bmax], found by thick-restart Lanczos on T_d(z(B)); the final
+// Rayleigh-Ritz step is done in a Hermitian operator R with R^2 = B (H_w: R = Q, B = Q^2, which separates +lambda from
+// -lambda) or R = B (D_ov: one chirality sector of D_ov^+ D_ov).  All callbacks enqueue on ctx->stream.
+struct LanczosOp {
+    double bmax = 1.0;
+    std::function<int(const double2* in, double2* out, double2* scratch)> base;                       // out = B in
+    std::function<int(const Filter& f, const double2* in, double2* out, double2* t1, double2* tq)> filter;  // out = T_d(z(B)) in
+    std::function<int(const double2* in, double2* out, double2* scratch)> rr;                         // out = R in
+    std::function<int(double2* v, double2* scratch)> start;                                           // project the start vector (may be empty)
+    std::function<double(double theta_min)> edge0;                                                    // first guess of the filter edge a
+};
+
+// out = T_d(z(B)) in for any base operator, three-term recurrence with separate BLAS-1 passes (used where one B costs
+// hundreds of Wilson launches, so the two extra streaming passes per term do not matter).  Same buffer rotation as
+// apply_filter: T_j lives in `out` when j has the parity of d, else in t1.
+static int generic_filter(ov_ctx* ctx, const LanczosOp& op, const Filter& f, const double2* in, double2* out, double2* t1,
+                          double2* tq, double2* scratch) {
+    const double w = f.b - f.a, cs = (f.a + f.b) / w;
+    auto buf = [&](int j) { return ((j & 1) == (f.d & 1)) ? out : t1; };
+    OV_TRY(op.base(in, tq, scratch));
+    OV_TRY(launch_axpby(ctx, 2.0 / w, tq, -cs, in, buf(1)));                       // T_1 = z(B) in
+    for (int j = 2; j <= f.d; j++) {
+        const double2* cur = buf(j - 1);
+        const double2* prev = (j == 2) ? in : buf(j - 2);
+        OV_TRY(op.base(cur, tq, scratch));
+        OV_TRY(launch_axpbypcz(ctx, 4.0 / w, tq, -2.0 * cs, cur, -1.0, prev, buf(j)));   // T_j = 2 z T_{j-1} - T_{j-2}
     }
     return OV_OK;
 }
@@ -124,12 +156,10 @@ extern "C" int ov_lanczos_stats(const ov_ctx* ctx, double* out_host) {
     return OV_OK;
 }
 
-extern "C" int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_restarts, int cheb_order, int subspace,
-                                   void* V_out_dev, double* lambda_out_host, double* resid_out_host) {
-    if (!ctx) return OV_EINVAL;
-    if (k < 1 || !(tol > 0) || max_restarts < 1 || cheb_order < 1 || !V_out_dev || !lambda_out_host || !resid_out_host)
-        return fail(ctx, OV_EINVAL, "bad argument to ov_lanczos_lowmodes");
-    if (!(ctx->norm > 0)) return fail(ctx, OV_ESTATE, "ov_set_polynomial (norm) has not been called");
+// Thick-restart Lanczos driver shared by the H_w and the D_ov low-mode routines (see LanczosOp).  nscratch extra spinors
+// beyond t1, tq are allocated for the callbacks (op.base / op.rr get the first one).
+static int lanczos_driver(ov_ctx* ctx, const LanczosOp& op, int k, double tol, int max_restarts, int cheb_order, int subspace,
+                          void* V_out_dev, double* lambda_out_host, double* resid_out_host) {
     const size_t n = spinor_elems(ctx), bytes = n * sizeof(double2);
     const long long dim = (long long)n;
     const int keep = k + std::max(8, k / 4);                    // wanted + buffer kept at every restart
@@ -138,17 +168,17 @@ extern "C" int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_resta
     if (m < m_min) m = m_min;
     if ((long long)m >= dim) return fail(ctx, OV_EINVAL, "subspace %d too large for dimension %lld", m, dim);
     if ((size_t)m * kRotTileBytesPerVector > 220 * 1024) m = (int)(220 * 1024 / kRotTileBytesPerVector);
-    {   // fit the pool into free memory: vectors k..m of the basis + 2 scratch (+ 2 GB head room for the workspaces)
+    {   // fit the pool into free memory: vectors k..m of the basis + 3 scratch (+ 2 GB head room for the workspaces)
         size_t free_b = 0, total_b = 0;
         OV_CUDA(ctx, cudaMemGetInfo(&free_b, &total_b));
         const size_t head = (size_t)2 << 30;
-        const long long fit = free_b > head ? (long long)((free_b - head) / bytes) - 4 : 0;   // pool vectors available
+        const long long fit = free_b > head ? (long long)((free_b - head) / bytes) - 5 : 0;   // pool vectors available
         if (subspace <= 0 && (long long)(m + 1 - k) > fit) m = (int)(fit + k - 1);
         if (m < m_min) return fail(ctx, OV_ENOMEM, "lanczos: %d basis vectors do not fit in free device memory", m_min + 1);
     }
 
-    double2* pool = nullptr;  // basis vectors k..m, then 2 scratch
-    const size_t npool = (size_t)(m + 1 - k) + 2;
+    double2* pool = nullptr;  // basis vectors k..m, then 3 scratch
+    const size_t npool = (size_t)(m + 1 - k) + 3;
     OV_CUDA(ctx, cudaMalloc(&pool, bytes * npool));
     double2 *d_C = nullptr, *d_St = nullptr;
     if (cudaMalloc(&d_C, (size_t)(m + 1) * sizeof(double2)) != cudaSuccess ||
@@ -160,6 +190,7 @@ extern "C" int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_resta
     const Basis W{(double2*)V_out_dev, k, pool, n};
     double2* t1 = pool + (size_t)(m + 1 - k) * n;
     double2* tq = t1 + n;
+    double2* t2 = tq + n;
 
     auto normalise = [&](double2* v, double* nrm) -> int {
         double s;
@@ -168,9 +199,10 @@ extern "C" int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_resta
         return launch_scale(ctx, 1.0 / *nrm, v);
     };
 
-    // ---- phase 0: a few plain Lanczos steps on A = Q^2 for an upper bound on lambda_min^2
+    // ---- phase 0: a few plain Lanczos steps on the base operator B for an upper bound on its lowest eigenvalue
     random_fill_kernel<<<(unsigned)((dim + 255) / 256), 256, 0, ctx->stream>>>(W.vec(0), dim, 0x1111628800ull);
     ctx->launches++;
+    if (op.start) OV_TRY(op.start(W.vec(0), t2));
     double nrm;
     OV_TRY(normalise(W.vec(0), &nrm));
     double theta_min;
@@ -179,12 +211,9 @@ extern "C" int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_resta
         std::vector<double2> T((size_t)m0 * m0, make_double2(0, 0)), S;
         std::vector<double> th;
         std::vector<double2> c;
-        const double inv = 1.0 / ctx->norm;
         for (int j = 0; j < m0; j++) {
             double2* u = W.vec(j + 1);
-            Epilogue e1; e1.s = inv;
-            OV_TRY(launch_wilson(ctx, W.vec(j), tq, e1));
-            OV_TRY(launch_wilson(ctx, tq, u, e1));
+            OV_TRY(op.base(W.vec(j), u, t2));
             OV_TRY(cgs_pass(ctx, W, j + 1, u, d_C, c));
             double alpha = c[j].x;
             OV_TRY(cgs_pass(ctx, W, j + 1, u, d_C, c));
@@ -196,7 +225,7 @@ extern "C" int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_resta
         host_eigh(m0, T, th, S);
         theta_min = std::max(th[0], 1e-12);
     }
-    Filter f{cheb_order, std::min(4.0 * theta_min, 0.5), 1.0};
+    Filter f{cheb_order, op.edge0(theta_min), op.bmax};
 
     std::vector<double2> T((size_t)m * m, make_double2(0, 0)), S, c;
     std::vector<double> th;
@@ -213,7 +242,7 @@ extern "C" int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_resta
         ctx->lanczos_stats = {(double)(restart + 1), (double)filter_applies, 0.0, f.a, (double)widenings, (double)m};
         for (int j = l; j < m; j++) {
             double2* u = W.vec(j + 1);
-            OV_TRY(apply_filter(ctx, f, W.vec(j), u, t1, tq));
+            OV_TRY(op.filter(f, W.vec(j), u, t1, tq));
             filter_applies++;
             OV_TRY(cgs_pass(ctx, W, j + 1, u, d_C, c));
             double alpha = c[j].x;
@@ -259,12 +288,12 @@ extern "C" int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_resta
             return OV_OK;
         };
         if (!refined_filter) {
-            // completeness guard: the amplified window [0, f.a) of Q^2 must hold the whole kept set.  If the keep-th Ritz
+            // completeness guard: the amplified window [0, f.a) of B must hold the whole kept set.  If the keep-th Ritz
             // value is not amplified (|theta| <= 1: it sits in the damped interval, so modes below lambda_k may be hidden
             // there too), the first guess 4 theta_min was too tight -- widen the window and start again.
-            if (std::fabs(th[kept[keep - 1]]) <= 1.0 + 1e-6 && f.a < 0.9 && widenings < 12) {
+            if (std::fabs(th[kept[keep - 1]]) <= 1.0 + 1e-6 && f.a < 0.9 * op.bmax && widenings < 12) {
                 widenings++;
-                OV_TRY(restart_with_edge(std::min(2.0 * f.a, 0.9)));
+                OV_TRY(restart_with_edge(std::min(2.0 * f.a, 0.9 * op.bmax)));
                 continue;
             }
             // tighten the filter edge to just above the kept set, restart the Krylov space from the Ritz vectors
@@ -276,12 +305,11 @@ extern "C" int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_resta
             }
         }
         if (conv) {
-            // Rayleigh-Ritz in Q on span(W[0..keep)): M = Y^+ Q Y
+            // Rayleigh-Ritz in R on span(W[0..keep)): M = Y^+ R Y
             std::vector<double2> M((size_t)keep * keep), SM;
             std::vector<double> mu;
-            Epilogue eq; eq.s = 1.0 / ctx->norm;
             for (int j = 0; j < keep; j++) {
-                OV_TRY(launch_wilson(ctx, W.vec(j), tq, eq));
+                OV_TRY(op.rr(W.vec(j), tq, t2));
                 OV_TRY(basis_dots(ctx, W, keep, tq));
                 c.resize(keep);
                 OV_TRY(fetch_results(ctx, keep, c.data()));
@@ -306,8 +334,8 @@ extern "C" int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_resta
                 double2* v = W.vec(i);
                 double nv;
                 OV_TRY(normalise(v, &nv));
-                Epilogue er; er.s = 1.0 / ctx->norm; er.A1 = v; er.a1 = -mu[order[i]];
-                OV_TRY(launch_wilson(ctx, v, tq, er));
+                OV_TRY(op.rr(v, tq, t2));
+                OV_TRY(launch_axpy(ctx, make_double2(-mu[order[i]], 0.0), v, tq));
                 double r2;
                 OV_TRY(norm2_host(ctx, tq, &r2));
                 lambda_out_host[i] = mu[order[i]];
@@ -358,4 +386,69 @@ extern "C" int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_resta
     OV_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     if (rc_final != OV_OK) return fail(ctx, OV_ENOCONV, "lanczos: residual above tol after %d restarts", max_restarts);
     return OV_OK;
+}
+
+extern "C" int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_restarts, int cheb_order, int subspace,
+                                   void* V_out_dev, double* lambda_out_host, double* resid_out_host) {
+    if (!ctx) return OV_EINVAL;
+    if (k < 1 || !(tol > 0) || max_restarts < 1 || cheb_order < 1 || !V_out_dev || !lambda_out_host || !resid_out_host)
+        return fail(ctx, OV_EINVAL, "bad argument to ov_lanczos_lowmodes");
+    if (!(ctx->norm > 0)) return fail(ctx, OV_ESTATE, "ov_set_polynomial (norm) has not been called");
+    LanczosOp op;
+    op.bmax = 1.0;                                     // B = Q^2, R = Q
+    const double inv = 1.0 / ctx->norm;
+    op.base = [ctx, inv](const double2* in, double2* out, double2* scratch) -> int {
+        Epilogue e1; e1.s = inv;
+        OV_TRY(launch_wilson(ctx, in, scratch, e1));
+        return launch_wilson(ctx, scratch, out, e1);
+    };
+    op.filter = [ctx](const Filter& f, const double2* in, double2* out, double2* t1, double2* tq) -> int {
+        return apply_filter(ctx, f, in, out, t1, tq);
+    };
+    op.rr = [ctx, inv](const double2* in, double2* out, double2*) -> int {
+        Epilogue eq; eq.s = inv;
+        return launch_wilson(ctx, in, out, eq);
+    };
+    op.edge0 = [](double theta_min) { return std::min(4.0 * theta_min, 0.5); };
+    return lanczos_driver(ctx, op, k, tol, max_restarts, cheb_order, subspace, V_out_dev, lambda_out_host, resid_out_host);
+}
+
+// Low modes of the overlap operator ("computing the low lying spectrum of the overlap
+// operator", :81 "Arnoldi ... Chebyshev acceleration ... Chebyshev order of 12").  Reading G20: the modes are
+// eigenpairs of A = D_ov(0)^+ D_ov(0) = 2 + gamma5 S + S gamma5, computed in ONE chirality sector s, where
+//     A_s x = 2 x + (s + gamma5) sign(H_w) x          (one sign per application, spectrum in [0, 4(1+delta)])
+// is non-degenerate; the other sector holds the same non-zero levels.  The same thick-restart driver as for H_w, with
+// B = R = A_s and the Chebyshev filter built from whole applications of A_s.
+extern "C" int ov_lanczos_dov_lowmodes(ov_ctx* ctx, int chirality, int k, double tol, int max_restarts, int cheb_order,
+                                       int subspace, void* W_out_dev, double* mu_out_host, double* resid_out_host) {
+    if (!ctx) return OV_EINVAL;
+    if ((chirality != 1 && chirality != -1) || k < 1 || !(tol > 0) || max_restarts < 1 || cheb_order < 1 || !W_out_dev ||
+        !mu_out_host || !resid_out_host)
+        return fail(ctx, OV_EINVAL, "bad argument to ov_lanczos_dov_lowmodes");
+    if (ctx->order < 0) return fail(ctx, OV_ESTATE, "ov_set_polynomial has not been called");
+    for (int i = 0; i <= 5; i++) {                     // the sign's workspaces, before the driver sizes its pool to free memory
+        double2* w;
+        OV_TRY(workspace(ctx, i, &w));
+    }
+    LanczosOp op;
+    op.bmax = 4.2;                                     // (1 + |S|)^2 with |S| <= 1 + delta, delta < 0.02
+    auto sector = [ctx, chirality](const double2* in, double2* out, double2* scratch) -> int {
+        OV_TRY(apply_sign(ctx, in, scratch));
+        return launch_chiral_combine(ctx, 2.0, in, chirality, scratch, out);
+    };
+    op.base = sector;
+    op.rr = sector;
+    // the filter needs one more scratch spinor than the driver hands over: workspace 5 (apply_sign uses 0-4)
+    const LanczosOp* self = &op;
+    op.filter = [ctx, self](const Filter& f, const double2* in, double2* out, double2* t1, double2* tq) -> int {
+        double2* scratch;
+        OV_TRY(workspace(ctx, 5, &scratch));
+        return generic_filter(ctx, *self, f, in, out, t1, tq, scratch);
+    };
+    op.start = [ctx, chirality](double2* v, double2* scratch) -> int {            // v <- (1 + s gamma5) v
+        OV_TRY(launch_copy(ctx, v, scratch));
+        return launch_chiral_combine(ctx, 0.0, nullptr, chirality, scratch, v);
+    };
+    op.edge0 = [](double theta_min) { return std::max(4.0 * theta_min, 0.2); };
+    return lanczos_driver(ctx, op, k, tol, max_restarts, cheb_order, subspace, W_out_dev, mu_out_host, resid_out_host);
 }

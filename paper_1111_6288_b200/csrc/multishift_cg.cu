@@ -2,6 +2,12 @@
 // PAPER.md:85; O8/G10).  One Krylov space serves all shifts sigma_i = m_i^2/(1 - m_i^2/4).
 // Host loop, device vectors; two host synchronisations per iteration (the scalars (p,q) and (r,r)),
 // negligible next to the ~2(2n+1) Wilson launches inside each A.
+//
+// Deflation (SURVEY 8f rank 2; PAPER.md:45 "we use deflation to help speed up the calculation", :81): with orthonormal
+// eigenpairs (mu_j, w_j) of A handed over by ov_set_deflation,
+//     x_i = sum_j w_j (w_j^+ b) / (mu_j + sigma_i)  +  CG solution for the projected source b - W W^+ b,
+// the CG stopping at |r| <= tol |b| (the full source).  The w_j must be eigenvectors of the A this routine applies to
+// within tol (include/ov.h): the true residuals returned at the end are computed with the full b and x_i and show it.
 #include <algorithm>
 #include <cmath>
 #include <numeric>
@@ -53,6 +59,17 @@ static std::vector<double> truncation_table(const std::vector<double>& c, double
 
 using namespace ov;
 
+extern "C" int ov_set_deflation(ov_ctx* ctx, const void* W_dev, const double* mu_host, int k) {
+    if (!ctx) return OV_EINVAL;
+    if (k < 0 || k > 1024 || (k > 0 && (!W_dev || !mu_host))) return fail(ctx, OV_EINVAL, "bad argument to ov_set_deflation");
+    for (int i = 0; i < k; i++)
+        if (!(mu_host[i] > -1e-6) || !std::isfinite(mu_host[i]))
+            return fail(ctx, OV_EINVAL, "deflation eigenvalue %d = %g: A = D^+ D is positive semi-definite", i, mu_host[i]);
+    ctx->Wdefl = k > 0 ? (const double2*)W_dev : nullptr;
+    ctx->mu_defl.assign(mu_host, mu_host + k);
+    return OV_OK;
+}
+
 extern "C" int ov_multishift_cg(ov_ctx* ctx, const double* masses_host, int nmass, const void* b_, void* x_,
                                 double tol, int maxiter, int* iters_out, double* relres_out) {
     if (!ctx) return OV_EINVAL;
@@ -85,18 +102,38 @@ extern "C" int ov_multishift_cg(ov_ctx* ctx, const double* masses_host, int nmas
     double2* q = r + n;
     double2* tmp = q + n;
 
-    for (int i = 0; i < nmass; i++) {
-        OV_TRY(launch_zero(ctx, x + (size_t)i * n));
-        OV_TRY(launch_copy(ctx, b, p[i]));
-    }
-    OV_TRY(launch_copy(ctx, b, r));
     double rr;
-    OV_TRY(norm2_host(ctx, r, &rr));
-    const double bnorm = std::sqrt(rr);
+    OV_TRY(norm2_host(ctx, b, &rr));
+    const double bnorm = std::sqrt(rr);   // every tolerance below is relative to the FULL source
     if (bnorm == 0.0) {
+        for (int i = 0; i < nmass; i++) OV_TRY(launch_zero(ctx, x + (size_t)i * n));
         if (iters_out) *iters_out = 0;
         if (relres_out) for (int i = 0; i < nmass; i++) relres_out[i] = 0.0;
         return OV_OK;
+    }
+    // deflation: r = b - W (W^+ b); the deflated part of every solution is added at the end
+    const int kd = (int)ctx->mu_defl.size();
+    std::vector<double2> cdefl(kd);
+    double2* d_cd = nullptr;
+    struct FreeC { double2*& p; ~FreeC() { cudaFree(p); } } guard_c{d_cd};
+    if (kd > 0) {
+        OV_CUDA(ctx, cudaMalloc(&d_cd, (size_t)kd * sizeof(double2)));
+        OV_TRY(launch_multi_dot(ctx, ctx->Wdefl, n, kd, b));
+        OV_TRY(fetch_results(ctx, kd, cdefl.data()));
+        std::vector<double2> neg(kd);
+        for (int j = 0; j < kd; j++) neg[j] = make_double2(-cdefl[j].x, -cdefl[j].y);
+        OV_CUDA(ctx, cudaMemcpyAsync(d_cd, neg.data(), kd * sizeof(double2), cudaMemcpyHostToDevice, ctx->stream));
+        OV_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        MultiAxpyOuts o;
+        o.out[0] = r; o.bscale[0] = 1.0;
+        OV_TRY(launch_multi_axpy(ctx, ctx->Wdefl, n, kd, 1, d_cd, b, o));
+        OV_TRY(norm2_host(ctx, r, &rr));
+    } else {
+        OV_TRY(launch_copy(ctx, b, r));
+    }
+    for (int i = 0; i < nmass; i++) {
+        OV_TRY(launch_zero(ctx, x + (size_t)i * n));
+        OV_TRY(launch_copy(ctx, r, p[i]));
     }
     // adaptive accuracy (ov_set_cg_adaptive): the application of A at iteration j may be off by eta_j ~ tol |b| / |r_j|
     std::vector<double> trunc;
@@ -121,8 +158,8 @@ extern "C" int ov_multishift_cg(ov_ctx* ctx, const double* masses_host, int nmas
     std::vector<char> active(nmass, 1);
     double a_old = 1.0, beta_old = 0.0;
     int it = 0;
-    bool converged = false;
-    while (it < maxiter) {
+    bool converged = std::sqrt(rr) <= tol * bnorm;   // e.g. a source inside the deflation space
+    while (!converged && it < maxiter) {
         // q = (A + s0) p_0   (position 0 = smallest shift)
         int order = ctx->order;
         bool f32 = false;
@@ -169,6 +206,20 @@ extern "C" int ov_multishift_cg(ov_ctx* ctx, const double* masses_host, int nmas
         if (std::sqrt(rr) <= tol * bnorm) { converged = true; break; }
     }
     if (iters_out) *iters_out = it;
+    if (kd > 0) {   // x_i += W (c / (mu + sigma_i))
+        std::vector<double2> coef(kd);
+        for (int i = 0; i < nmass; i++) {
+            for (int j = 0; j < kd; j++) {
+                const double d = 1.0 / (ctx->mu_defl[j] + sig[i]);
+                coef[j] = make_double2(cdefl[j].x * d, cdefl[j].y * d);
+            }
+            OV_CUDA(ctx, cudaMemcpyAsync(d_cd, coef.data(), kd * sizeof(double2), cudaMemcpyHostToDevice, ctx->stream));
+            OV_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+            MultiAxpyOuts o;
+            o.out[0] = x + (size_t)i * n; o.bscale[0] = 1.0;
+            OV_TRY(launch_multi_axpy(ctx, ctx->Wdefl, n, kd, 1, d_cd, x + (size_t)i * n, o));
+        }
+    }
     if (relres_out) {  // true residuals |b - (A + sigma_i) x_i| / |b|
         for (int i = 0; i < nmass; i++) {
             OV_TRY(apply_A(ctx, x + (size_t)i * n, tmp, q));

@@ -90,6 +90,10 @@ struct ov_ctx {
     double2* d_coef = nullptr;     // k complex: c = V^+ x
     int cap_k = 0;
 
+    // deflation space of the multi-shift CG (borrowed W, eigenpairs of A = D_ov^+ D_ov; ov_set_deflation)
+    const double2* Wdefl = nullptr;
+    std::vector<double> mu_defl;
+
     // workspaces
     double2* ws[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     float2* wsf[4] = {nullptr, nullptr, nullptr, nullptr};  // fp32 Clenshaw vectors
@@ -163,6 +167,9 @@ void host_eigh(int n, std::vector<double2>& A, std::vector<double>& w, std::vect
 // BLAS-1 on ABI spinors (n = 12 V complex)
 int launch_axpy(ov_ctx* ctx, double2 a, const double2* x, double2* y);                     // y += a x
 int launch_axpby(ov_ctx* ctx, double a, const double2* x, double b, const double2* y, double2* z, int nrhs = 1);  // z = a x + b y
+int launch_axpbypcz(ov_ctx* ctx, double a, const double2* x, double b, const double2* y, double c, const double2* w, double2* z);
+// out = ax x + (s + gamma5) y, s = +-1 (x may be null when ax = 0): chirality-sector algebra of D_ov^+ D_ov
+int launch_chiral_combine(ov_ctx* ctx, double ax, const double2* x, int s, const double2* y, double2* out);
 int launch_scale(ov_ctx* ctx, double a, double2* x);
 int launch_copy(ov_ctx* ctx, const double2* x, double2* y);
 int launch_zero(ov_ctx* ctx, double2* x);

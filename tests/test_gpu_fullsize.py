@@ -304,3 +304,78 @@ def test_adaptive_cg_16x32_vs_oracle_cg(ovp, cfg2, parity_log):
     finally:
         op.set_cg_adaptive(0)
         op.set_polynomial(ovp.chebyshev_coeffs(cfg.order, cfg.eps), cfg.eps, cfg.norm)
+
+
+# ------------------------------------------------------------------------------------------ deflation at size (8f rank 2)
+def test_deflated_cg_16x32_hard_workload(ovp, parity_log):
+    """D_ov low modes + deflated multi-mass CG on workloads.DEFLATION (16^3x32, smooth links, periodic time; PAPER.md:45
+    "deflation was shown to increase the convergence rate by a factor of 3-4").  The eigenpairs and the solution of the
+    lightest mass are re-checked with the ORACLE's operator; iterations must drop by >= 2."""
+    from oracle import deflation as dfl
+    cfg = wl.DEFLATION
+    bc = (1.0, 1.0, 1.0, 1.0)
+    U = wl.su3_links(cfg.dims, cfg.spread, wl.gauge_seed(cfg.index))
+    op = ovp.Overlap(cfg.dims, cfg.kappa, U, t_boundary=wl.DEFLATION_T_BOUNDARY)
+    op.set_polynomial(ovp.chebyshev_coeffs(10, 0.01), 0.01, cfg.norm)            # norm for the H_w eigensolver
+    V, lam, res, ok = op.lanczos_lowmodes(16, tol=1e-9, max_restarts=60, cheb_order=100)
+    assert ok
+    se = 0.95 * float(np.max(np.abs(lam)))
+    # delta ~ 1e-12 by eq. 2.2 (PAPER.md:37): the deflated part of x carries the defect 1 - sign^2 = O(delta) of the
+    # sector eigenvectors amplified by 1/(mu_0 + sigma_0) ~ 4e4, and must stay below tol = 1e-8 (include/ov.h, ov_set_deflation)
+    n = int(np.ceil(np.log(0.41 / 1e-12) / (2.1 * se)))
+    coef = ovp.chebyshev_coeffs(n, se * se)
+    op.set_polynomial(coef, se * se, cfg.norm)
+    op.set_smallspace(V, lam)
+    k = 12
+    Ws, mus = [], []
+    for s in (+1, -1):
+        W, mu, r, ok = op.lanczos_dov_lowmodes(s, k, tol=1e-9, max_restarts=60, cheb_order=12)
+        st = op.lanczos_stats()
+        assert ok and np.all(r <= 1e-9)
+        print(f"  D_ov low modes, chirality {s:+d}: mu = {np.array2string(np.sort(mu), precision=5)}; {st['restarts']} cycles, "
+              f"{st['filter_applies']} filter applies, order {n}, sqrt(eps) {se:.4f}")
+        Ws.append(W); mus.append(mu)
+    assert np.max(np.abs(np.sort(mus[0])[6:] - np.sort(mus[1])[6:])) <= 1e-7     # pairing of the non-zero levels
+    Vh = host(op, V)
+    with oracle.boundary(bc):                                                     # the oracle's A_s confirms two pairs per sector
+        sgn = lambda v: oracle.sign(cfg.dims, cfg.kappa, U, coef, se * se, cfg.norm, Vh, lam, v)
+        for s, W, mu in zip((+1, -1), Ws, mus):
+            Wh = host(op, W[:2].contiguous())
+            for i in range(2):
+                r = dfl.sector_op(sgn, s, Wh[i]) - mu[i] * Wh[i]
+                e = float(np.linalg.norm(r.ravel()))
+                parity_log(f"16^3x32 D_ov low mode {i} (chirality {s:+d}, mu = {mu[i]:.3e}): |A_s w - mu w| with the oracle's sign", e, 1e-8)
+                assert e <= 1e-8
+    Wd = torch.cat(Ws).contiguous()
+    mud = np.concatenate(mus)
+    b = wl.point_source(cfg.dims)
+    db = dev(op, b)
+    import time
+    t0 = time.time()
+    x_plain, it_plain, res_plain, ok1 = op.multishift_cg(list(cfg.masses), db, tol=1e-8, maxiter=5000)
+    t_plain = time.time() - t0
+    op.set_deflation(Wd, mud)
+    t0 = time.time()
+    x_defl, it_defl, res_defl, ok2 = op.multishift_cg(list(cfg.masses), db, tol=1e-8, maxiter=5000)
+    t_defl = time.time() - t0
+    op.set_deflation(None, None)
+    print(f"  multi-mass CG, 6 masses, tol 1e-8: plain {it_plain} iterations {t_plain:.1f} s, deflated (2 x {k} modes) "
+          f"{it_defl} iterations {t_defl:.1f} s; true residuals plain {res_plain.max():.2e}, deflated {res_defl.max():.2e}")
+    assert ok1 and ok2
+    assert np.all(res_plain <= 1.2e-8) and np.all(res_defl <= 1.2e-8)
+    parity_log(f"16^3x32 hard workload: CG iterations plain / deflated = {it_plain} / {it_defl} (gate: 2 deflated <= plain)",
+               2.0 * it_defl / it_plain, 1.0)
+    assert it_plain >= 2 * it_defl
+    for i in (0, len(cfg.masses) - 1):
+        e = rel(host(op, x_defl[i:i + 1].contiguous())[0], host(op, x_plain[i:i + 1].contiguous())[0])
+        parity_log(f"16^3x32 deflated vs plain solution, mass {cfg.masses[i]}", e, 1e-5)
+        assert e <= 1e-5
+    # the oracle's operator on the deflated solution of the lightest mass: |b - (A + sigma) x| / |b|
+    xh = host(op, x_defl[0:1].contiguous())[0]
+    with oracle.boundary(bc):
+        args = (cfg.dims, cfg.kappa, U, coef, se * se, cfg.norm, Vh, lam)
+        Ax = dfl.normal_op(lambda u: oracle.dov(*args, 0.0, u), xh)
+    sg = sigma_of_mass(cfg.masses[0])
+    e = float(np.linalg.norm((b - Ax - sg * xh).ravel()) / np.linalg.norm(b.ravel()))
+    parity_log("16^3x32 deflated solution, lightest mass: true residual with the ORACLE's D_ov", e, 2e-8)
+    assert e <= 2e-8

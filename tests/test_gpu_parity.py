@@ -447,6 +447,74 @@ def test_background_field_and_boundaries_api_vs_oracle(ovp, variant, t_boundary,
     assert rel(to_host(op12, op12.apply_hw(to_dev(op12, x))), ref12) <= TOL_HW
 
 
+# ------------------------------------------------------------------------------------------ D_ov low modes, deflated CG
+def test_dov_lowmodes_and_deflated_cg_4x4_vs_oracle(ovp, parity_log):
+    """SURVEY 8f rank 2 on the oracle's hard 4^4 lattice (smooth links, periodic time: 6 near-zero
+    modes of D_ov^+ D_ov per chirality sector).  (a) ov_lanczos_dov_lowmodes per sector = the dense eigenpairs of the
+    exact A; (b) the deflated multi-mass CG = the oracle's deflated CG (same iterations +-1, solutions) and the dense
+    direct solve; (c) deflation cuts the iterations by > 3."""
+    from oracle import deflation as dfl
+    dims = (4, 4, 4, 4)
+    U = wl.su3_links(dims, 0.3, 41)
+    bc = (1.0, 1.0, 1.0, 1.0)
+    with oracle.boundary(bc):
+        w, Zv, _, _ = dense.eig_hw(dims, KAPPA, U)
+    A = dfl.dense_normal(w, Zv)
+    shape = (4, 4, 4, 4, 4, 3)
+    N = A.shape[0]
+    se = 0.9 * np.min(np.abs(w)) / NORM                     # the polynomial covers the whole spectrum of Q: no small space
+    n = int(np.ceil(np.log(0.41 / 1e-11) / (2.1 * se)))     # delta ~ 1e-11 by eq. 2.2 (PAPER.md:37)
+    coef = ovp.chebyshev_coeffs(n, se * se)
+    op = ovp.Overlap(dims, KAPPA, U, t_boundary="periodic")
+    op.set_polynomial(coef, se * se, NORM)
+    k = 6
+    Ws, mus = [], []
+    for s in (+1, -1):
+        W, mu, res, ok = op.lanczos_dov_lowmodes(s, k, tol=1e-10, max_restarts=60, cheb_order=12, subspace=30)
+        assert ok and np.all(res <= 1e-10)
+        mu_ref, _ = dfl.dense_sector_modes(A, s, k, shape)
+        err = float(np.max(np.abs(np.sort(mu) - mu_ref)))
+        parity_log(f"4^4 D_ov low modes, chirality {s:+d}: max |mu_i - dense mu_i| (mu in [{mu_ref[0]:.1e}, {mu_ref[-1]:.1e}])", err, 1e-9)
+        assert err <= 1e-9
+        Wh = to_host(op, W)
+        for i in range(k):                                   # the dense exact operator confirms each pair; chirality
+            v = Wh[i].reshape(-1)
+            assert np.linalg.norm(A @ v - mu[i] * v) <= 1e-8
+            assert rel(dfl.gamma5(Wh[i]), s * Wh[i]) <= 1e-10
+        Ws.append(W); mus.append(mu)
+    Wd = torch.cat(Ws).contiguous()
+    mud = np.concatenate(mus)
+    masses = [0.005, 0.02, 0.1]
+    sig = [sigma_of_mass(m) for m in masses]
+    b = wl.gaussian_source(dims, 43)
+    db = to_dev(op, b)
+    x_plain, it_plain, res_plain, ok1 = op.multishift_cg(masses, db, tol=1e-9, maxiter=2000)
+    op.set_deflation(Wd, mud)
+    x_defl, it_defl, res_defl, ok2 = op.multishift_cg(masses, db, tol=1e-9, maxiter=2000)
+    op.set_deflation(None, None)
+    assert ok1 and ok2 and np.all(res_plain <= 1e-8) and np.all(res_defl <= 1e-8)
+    # the oracle's deflated CG with the oracle's own (dense) modes and the oracle's polynomial D_ov
+    mu_p, W_p = dfl.dense_sector_modes(A, +1, k, shape)
+    mu_m, W_m = dfl.dense_sector_modes(A, -1, k, shape)
+    with oracle.boundary(bc):
+        args = (dims, KAPPA, U, coef, se * se, NORM, None, None)
+        Aor = lambda v: dfl.normal_op(lambda u: oracle.dov(*args, 0.0, u), v)
+        xs, it_ref, res_ref = dfl.deflated_multishift_cg(Aor, np.concatenate([W_p, W_m]), np.concatenate([mu_p, mu_m]),
+                                                         sig, b, 1e-9, 2000)
+    assert abs(it_defl - it_ref) <= 1
+    got = to_host(op, x_defl)
+    for i, sg in enumerate(sig):
+        e1 = rel(got[i], xs[i])
+        direct = np.linalg.solve(A + sg * np.eye(N), b.reshape(-1)).reshape(shape)
+        e2 = rel(got[i], direct)
+        parity_log(f"4^4 deflated multi-mass CG, mass {masses[i]}: vs oracle deflated CG ({it_defl} vs {it_ref} iterations)", e1, 1e-6)
+        parity_log(f"4^4 deflated multi-mass CG, mass {masses[i]}: vs dense direct solve with the exact sign", e2, 1e-6)
+        assert e1 <= 1e-6 and e2 <= 1e-6
+    parity_log(f"4^4 iterations plain / deflated = {it_plain} / {it_defl}: ratio (gate: >= 3, reported as 3/ratio <= 1)",
+               3.0 * it_defl / it_plain, 1.0)
+    assert it_plain >= 3 * it_defl
+
+
 # ------------------------------------------------------------------------------------------ degenerate cases
 def test_degenerate_inputs(ovp, cfg0):
     c = cfg0

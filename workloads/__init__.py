@@ -11,6 +11,8 @@ Canonical array conventions (reading G16):
 """
 from .generators import (  # noqa: F401
     CONFIGS,
+    DEFLATION,
+    DEFLATION_T_BOUNDARY,
     LatticeConfig,
     su3_links,
     unit_links,

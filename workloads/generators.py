@@ -159,3 +159,11 @@ CONFIGS = (
     LatticeConfig(4, (32, 32, 32, 64), 0.8, order=300, sqrt_eps=0.01, k=200, nsrc=1,
                   masses=(0.005, 0.01, 0.02, 0.04, 0.07, 0.1), name="32^3x64"),
 )
+
+
+# The workload of the deflation row: the random links of CONFIGS give D_ov^+ D_ov a
+# spectrum in [2.7, 4] (nothing to deflate), so this one is SMOOTH (small spread) and PERIODIC in time: the p = 0 modes of
+# the free overlap operator survive as 6 near-zero modes of D_ov^+ D_ov per chirality sector (condition number ~ 1e4-1e5
+# at the lightest mass), followed by the p = 2 pi / T shell -- the situation deflation is for.
+DEFLATION = LatticeConfig(5, (16, 16, 16, 32), 0.3, masses=(0.005, 0.01, 0.02, 0.04, 0.07, 0.1), name="16^3x32 smooth links, periodic t")
+DEFLATION_T_BOUNDARY = "periodic"
