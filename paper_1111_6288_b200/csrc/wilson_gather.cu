@@ -225,6 +225,7 @@ int launch_wilson_gather(ov_ctx* ctx, const double2* in, double2* out, const Epi
     return launch_gather_t<double2>(ctx, ctx->gauge, in, out, ep);
 }
 int launch_wilson_batch(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep, int nrhs) {
+    if (nrhs == 1) return launch_wilson(ctx, in, out, ep);   // single right-hand side: the context's kernel choice
     return launch_gather_t<double2>(ctx, ctx->gauge, in, out, ep, nrhs, (long long)spinor_elems(ctx));
 }
 int launch_wilson_gather_f32(ov_ctx* ctx, const float2* in, float2* out, const EpilogueF& ep) {

@@ -4,25 +4,19 @@
 //   out = s * G (in - kappa * hop(in)) + a1*A1 + a2*A2 + a3*A3          (Epilogue, ov_internal.h)
 //
 // Why: the gather kernel (variant 1) pulls 2.2-2.3 kB/site through the SM's L2 port for 960 B/site of HBM traffic and
-// sits at the L2 throughput cap.  Here every operand reaches the SM exactly once per tile through the TMA unit:
+// is bound there.  Here every operand reaches the SM exactly once per tile through the TMA unit:
 //   * the lattice is cut into pencils of 8 x 4 x 4 sites in (x,y,z); one CTA marches a pencil along t, one time slice
-//     (128 sites) per step;
-//   * ONE producer thread issues cp.async.bulk.tensor (5-D boxes over the planes layout [comp][t][z][y][x]) into
-//     shared memory: a ring of three interior spinor planes (t, t+1 and one in flight) and one DEDICATED slot per
-//     object of a slice -- the x / y / z halo faces (one-site-thick boxes; wrapped coordinates are separate boxes by
-//     construction) and the link chunks of the four directions (+ the one-site-thick face of backward links).  Every slot
-//     has an mbarrier full/empty pair; the producer polls the empty barriers (test_wait) and refills whichever slot was
-//     released first, so no issue order has to be guessed;
-//   * EIGHT consumer warps in two groups share the staged data, one site per thread in each group:
-//       group A (warps 0-3): own-site term, x and y hops  ->  partial accumulator handed over through shared memory;
-//       group B (warps 4-7): starts from A's partial, z and t hops, epilogue, coalesced 16-byte stores.
-//     A runs about one slice ahead of B; each object is in use for less than half a slice time and is refilled during the
-//     rest, which is why single slots suffice.  The forward t neighbour is the next interior plane (it later becomes the
-//     own plane); the backward t hop U_t(x-t)^+ (1+gamma_t) psi(x-t) is carried in B's registers from the previous step.
-//     The additions happen in the same order as in the gather kernel, so the two kernels agree to the last bit except
-//     where the compiler contracts an FMA differently.
-//   * epilogue operands are read by group B from global memory at the output site; the producer prefetches their boxes
-//     into L2 (cp.async.bulk.prefetch.tensor) two slices ahead.
+//     (128 sites = 4 consumer warps, one site per thread) per step;
+//   * ONE producer thread issues cp.async.bulk.tensor (5-D boxes over the planes layout [comp][t][z][y][x]) into three
+//     shared-memory rings guarded by mbarrier full/empty pairs: spinor interior planes (3 slots: t, t+1 and one in
+//     flight), spinor halo faces of the current slice (6 one-site-thick boxes, wrapped coordinates are separate boxes
+//     by construction; 2 slots), and link chunks (one direction of one slice + the one-site-thick halo of backward
+//     links; 4 slots).  The producer runs about one slice ahead of the consumers, so ~140 kB are in flight per SM with
+//     no register spent on them and no __syncthreads between loading and computing;
+//   * consumers read neighbours and links from shared memory only (forward t neighbour = the next interior plane, which
+//     later becomes the site's own plane; the backward t hop U_t(x-t)^+ (1+gamma_t) psi(x-t) is carried in registers
+//     from the previous step), do the same arithmetic in the same order as the gather kernel (results are bit-identical),
+//     and store the result with coalesced 16-byte stores.
 // L2->SM traffic per site: 192 (own) + 240 (halo) + 576 (links) + 72 (halo links) = 1080 B instead of ~2200.
 //
 // Needs the planes layout and X % 8 == 0, Y % 4 == 0, Z % 4 == 0; other shapes use the gather kernel.
@@ -38,27 +32,18 @@ namespace ov {
 namespace tma {
 
 constexpr int BX = 8, BY = 4, BZ = 4;           // tile of one time slice
-constexpr int SITES = BX * BY * BZ;             // 128 = 4 warps per consumer group
-constexpr int NGRP = SITES / 32;                // warps per consumer group
-constexpr int NCONS = 2 * NGRP;                 // consumer warps (groups A and B)
-constexpr int THREADS = (NCONS + 4) * 32;       // + the producer's warpgroup (one warp issues, three exit at once): three
-                                                // aligned warpgroups, so that setmaxnreg can move registers to the consumers
-constexpr int REG_CONSUMER = 232, REG_PRODUCER = 40;   // 128 * (2 * 232 + 40) = 64512 <= 65536
-constexpr int SI = 3;                           // interior planes in the ring
+constexpr int SITES = BX * BY * BZ;             // 128 = 4 consumer warps
+constexpr int NCONS = SITES / 32;               // consumer warps
+constexpr int THREADS = SITES + 32;             // + 1 producer warp
+constexpr int SI = 3, SH = 2, SL = 4;           // ring depths: interior planes, halo sets, link chunks
 constexpr int I_BYTES = SITES * 12 * 16;        // 24576
 constexpr int FX = BY * BZ, FY = BX * BZ, FZ = BX * BY;   // face sites: 16, 32, 32
-constexpr int HX_BYTES = 2 * 12 * FX * 16, HY_BYTES = 2 * 12 * FY * 16, HZ_BYTES = 2 * 12 * FZ * 16;   // minus face, plus face
-constexpr int P_BYTES = SITES * 12 * 16;        // group A's partial accumulators
-template <int NE> struct LBytes {               // link chunk = the tile's links of one direction + the face of backward links
-    static constexpr int x = (SITES + FX) * NE * 16, y = (SITES + FY) * NE * 16, z = (SITES + FZ) * NE * 16, t = SITES * NE * 16;
-};
-// single-slot objects and their barrier index (full at 2*o, empty at 2*o + 1 after the interior ring's barriers)
-enum Obj { HX = 0, HY, HZ, LX, LY, LZ, LT, NOBJ };
-constexpr int NBAR = 2 * SI + 2 * NOBJ + 2 * NGRP;
-template <int NE> constexpr size_t smem_bytes() {
-    return (size_t)SI * I_BYTES + HX_BYTES + HY_BYTES + HZ_BYTES + LBytes<NE>::x + LBytes<NE>::y + LBytes<NE>::z + LBytes<NE>::t +
-           P_BYTES + 8 * NBAR;
-}
+constexpr int H_ELEMS = 12 * (2 * FX + 2 * FY + 2 * FZ);  // 1920 double2
+constexpr int H_BYTES = H_ELEMS * 16;           // 30720
+// offsets (double2) of the six faces inside a halo slot: x-, x+, y-, y+, z-, z+
+constexpr int HOFF_XM = 0, HOFF_XP = 12 * FX, HOFF_YM = 24 * FX, HOFF_YP = 24 * FX + 12 * FY,
+              HOFF_ZM = 24 * FX + 24 * FY, HOFF_ZP = 24 * FX + 24 * FY + 12 * FZ;
+template <int NE> struct LSlot { static constexpr int bytes = (SITES + 32) * NE * 16; };   // main box + the largest halo face
 
 struct Maps {               // tensor maps of one spinor array or of the gauge field (box shapes differ)
     CUtensorMap main, fx, fy, fz;
@@ -67,7 +52,6 @@ struct Maps {               // tensor maps of one spinor array or of the gauge f
 struct Args {
     Maps in;                // spinor: 5-D (2X, Y, Z, T, 12) doubles
     Maps gauge;             // links:  5-D (2X, Y, Z, T, 4*NE) doubles
-    CUtensorMap op[3];      // main-box maps of the epilogue operands (L2 prefetch only)
     double2* out;
     const double2* A1;
     const double2* A2;
@@ -106,26 +90,17 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
         "WAIT_DONE:\n"
         "}\n" ::"r"(bar), "r"(parity) : "memory");
 }
-__device__ __forceinline__ bool mbar_test(unsigned bar, unsigned parity) {
-    unsigned ok;
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n"
-        "selp.u32 %0, 1, 0, p;\n"
-        "}\n" : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
-    return ok != 0;
-}
 __device__ __forceinline__ void tma_load_5d(unsigned dst, const CUtensorMap* map, unsigned bar, int c0, int c1, int c2,
                                             int c3, int c4) {
     asm volatile(
         "cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6, %7}], [%2];"
         ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4) : "memory");
 }
-__device__ __forceinline__ void tma_prefetch_5d(const CUtensorMap* map, int c0, int c1, int c2, int c3, int c4) {
-    asm volatile("cp.async.bulk.prefetch.tensor.5d.L2.global.tile [%0, {%1, %2, %3, %4, %5}];"
-                 ::"l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4) : "memory");
-}
+
+// ring bookkeeping: fill number n lives in slot n % S and is that slot's (n / S)-th use
+template <int S> __device__ __forceinline__ unsigned slot_of(unsigned n) { return n % S; }
+template <int S> __device__ __forceinline__ unsigned full_parity(unsigned n) { return (n / S) & 1u; }
+template <int S> __device__ __forceinline__ unsigned empty_parity(unsigned n) { return ((n / S) & 1u) ^ 1u; }
 
 struct Item {
     int x0, y0, z0, t0;
@@ -165,15 +140,6 @@ __device__ __forceinline__ void hop_smem(double2* acc, const double2* pn, int ns
     reconstruct_add<MU, SIGMA>(acc, g, ph);
 }
 
-// the fill sequence of one staged object as the producer sees it: fill number f belongs to the CTA's j-th work item and
-// is the u-th of that item's `per` fills
-struct Seq {
-    int j = 0, u = 0, per = 0, nitem = 0;
-    unsigned f = 0;
-    __device__ __forceinline__ bool done() const { return j >= nitem; }
-    __device__ __forceinline__ void next() { f++; if (++u == per) { u = 0; j++; } }
-};
-
 }  // namespace tma
 
 using namespace tma;
@@ -182,246 +148,187 @@ using namespace tma;
 template <int RECON, int NA>
 __global__ void __launch_bounds__(THREADS, 1) wilson_tma_kernel(const __grid_constant__ Args a) {
     constexpr int NE = RECON / 2;
-    using LB = LBytes<NE>;
+    constexpr int L_BYTES = LSlot<NE>::bytes;
     extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char* sI = smem;
-    unsigned char* sHX = sI + SI * I_BYTES;
-    unsigned char* sHY = sHX + HX_BYTES;
-    unsigned char* sHZ = sHY + HY_BYTES;
-    unsigned char* sLX = sHZ + HZ_BYTES;
-    unsigned char* sLY = sLX + LB::x;
-    unsigned char* sLZ = sLY + LB::y;
-    unsigned char* sLT = sLZ + LB::z;
-    unsigned char* sP = sLT + LB::t;
-    unsigned long long* bars = (unsigned long long*)(sP + P_BYTES);
+    unsigned char* sH = sI + SI * I_BYTES;
+    unsigned char* sL = sH + SH * H_BYTES;
+    unsigned long long* bars = (unsigned long long*)(sL + SL * L_BYTES);
+    // barrier indices: fullI[SI], emptyI[SI], fullH[SH], emptyH[SH], fullL[SL], emptyL[SL]
     const unsigned bar0 = smem_u32(bars);
     auto fullI = [&](unsigned s) { return bar0 + 8u * s; };
     auto emptyI = [&](unsigned s) { return bar0 + 8u * (SI + s); };
-    auto fullO = [&](int o) { return bar0 + 8u * (2 * SI + 2 * o); };
-    auto emptyO = [&](int o) { return bar0 + 8u * (2 * SI + 2 * o + 1); };
-    auto partFull = [&](int w) { return bar0 + 8u * (2 * SI + 2 * NOBJ + w); };
-    auto partEmpty = [&](int w) { return bar0 + 8u * (2 * SI + 2 * NOBJ + NGRP + w); };
+    auto fullH = [&](unsigned s) { return bar0 + 8u * (2 * SI + s); };
+    auto emptyH = [&](unsigned s) { return bar0 + 8u * (2 * SI + SH + s); };
+    auto fullL = [&](unsigned s) { return bar0 + 8u * (2 * SI + 2 * SH + s); };
+    auto emptyL = [&](unsigned s) { return bar0 + 8u * (2 * SI + 2 * SH + SL + s); };
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) {
         for (unsigned s = 0; s < SI; s++) { mbar_init(fullI(s), 1); mbar_init(emptyI(s), NCONS); }
-        for (int o = 0; o < NOBJ; o++) { mbar_init(fullO(o), 1); mbar_init(emptyO(o), NGRP); }
-        for (int w = 0; w < NGRP; w++) { mbar_init(partFull(w), 1); mbar_init(partEmpty(w), 1); }
+        for (unsigned s = 0; s < SH; s++) { mbar_init(fullH(s), 1); mbar_init(emptyH(s), NCONS); }
+        for (unsigned s = 0; s < SL; s++) { mbar_init(fullL(s), 1); mbar_init(emptyL(s), NCONS); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
 
-    const int my_items = (a.nitems - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
-
-    if (warp >= NCONS) {
+    if (warp == NCONS) {
         // =============================================================== producer: one thread issues every TMA load
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REG_PRODUCER));
-        if (warp != NCONS || lane != 0) return;
-        Seq qI, q[NOBJ];
-        qI.per = a.Lt + 2; qI.nitem = my_items;                 // planes t0-1, t0 .. t0+Lt-1, t0+Lt
-        for (int o = 0; o < NOBJ; o++) { q[o].per = (o == LT) ? a.Lt + 1 : a.Lt; q[o].nitem = my_items; }   // LT: + the slice below
-        auto item_of = [&](int j) { return decode_item(a, (int)blockIdx.x + j * (int)gridDim.x); };
-        auto wrap = [&](int t) { return t < 0 ? t + a.T : (t >= a.T ? t - a.T : t); };
-        int remaining = 1 + NOBJ;
-        while (remaining > 0) {
-            bool progress = false;
-            remaining = 0;
-            if (!qI.done()) {
-                remaining++;
-                const unsigned s = qI.f % SI;
-                if (mbar_test(emptyI(s), ((qI.f / SI) & 1u) ^ 1u)) {
-                    const Item w = item_of(qI.j);
-                    const int t = wrap(w.t0 - 1 + qI.u);
-                    mbar_expect_tx(fullI(s), I_BYTES);
-                    tma_load_5d(smem_u32(sI + s * I_BYTES), &a.in.main, fullI(s), 2 * w.x0, w.y0, w.z0, t, 0);
-                    if (NA >= 1 && qI.u >= 1 && qI.u <= a.Lt) {   // an own plane: pull its epilogue operands into L2
-                        tma_prefetch_5d(&a.op[0], 2 * w.x0, w.y0, w.z0, t, 0);
-                        if (NA >= 2) tma_prefetch_5d(&a.op[1], 2 * w.x0, w.y0, w.z0, t, 0);
-                        if (NA >= 3) tma_prefetch_5d(&a.op[2], 2 * w.x0, w.y0, w.z0, t, 0);
-                    }
-                    qI.next();
-                    progress = true;
-                }
+        if (lane != 0) return;
+        unsigned nI = 0, nH = 0, nL = 0;
+        auto fill_I = [&](const Item& w, int t) {
+            const unsigned s = slot_of<SI>(nI);
+            mbar_wait(emptyI(s), empty_parity<SI>(nI));
+            mbar_expect_tx(fullI(s), I_BYTES);
+            tma_load_5d(smem_u32(sI + s * I_BYTES), &a.in.main, fullI(s), 2 * w.x0, w.y0, w.z0, t, 0);
+            nI++;
+        };
+        auto fill_H = [&](const Item& w, int t) {
+            const unsigned s = slot_of<SH>(nH);
+            mbar_wait(emptyH(s), empty_parity<SH>(nH));
+            mbar_expect_tx(fullH(s), H_BYTES);
+            const unsigned base = smem_u32(sH + s * H_BYTES);
+            const int xm = (w.x0 == 0) ? a.X - 1 : w.x0 - 1, xp = (w.x0 + BX == a.X) ? 0 : w.x0 + BX;
+            const int ym = (w.y0 == 0) ? a.Y - 1 : w.y0 - 1, yp = (w.y0 + BY == a.Y) ? 0 : w.y0 + BY;
+            const int zm = (w.z0 == 0) ? a.Z - 1 : w.z0 - 1, zp = (w.z0 + BZ == a.Z) ? 0 : w.z0 + BZ;
+            tma_load_5d(base + 16 * HOFF_XM, &a.in.fx, fullH(s), 2 * xm, w.y0, w.z0, t, 0);
+            tma_load_5d(base + 16 * HOFF_XP, &a.in.fx, fullH(s), 2 * xp, w.y0, w.z0, t, 0);
+            tma_load_5d(base + 16 * HOFF_YM, &a.in.fy, fullH(s), 2 * w.x0, ym, w.z0, t, 0);
+            tma_load_5d(base + 16 * HOFF_YP, &a.in.fy, fullH(s), 2 * w.x0, yp, w.z0, t, 0);
+            tma_load_5d(base + 16 * HOFF_ZM, &a.in.fz, fullH(s), 2 * w.x0, w.y0, zm, t, 0);
+            tma_load_5d(base + 16 * HOFF_ZP, &a.in.fz, fullH(s), 2 * w.x0, w.y0, zp, t, 0);
+            nH++;
+        };
+        auto fill_L = [&](const Item& w, int t, int mu) {
+            const unsigned s = slot_of<SL>(nL);
+            mbar_wait(emptyL(s), empty_parity<SL>(nL));
+            const unsigned base = smem_u32(sL + s * L_BYTES);
+            const int face = (mu == 0) ? FX : (mu == 1) ? FY : (mu == 2) ? FZ : 0;
+            mbar_expect_tx(fullL(s), (SITES + face) * NE * 16);
+            tma_load_5d(base, &a.gauge.main, fullL(s), 2 * w.x0, w.y0, w.z0, t, mu * NE);
+            if (mu == 0) {
+                const int xm = (w.x0 == 0) ? a.X - 1 : w.x0 - 1;
+                tma_load_5d(base + SITES * NE * 16, &a.gauge.fx, fullL(s), 2 * xm, w.y0, w.z0, t, mu * NE);
+            } else if (mu == 1) {
+                const int ym = (w.y0 == 0) ? a.Y - 1 : w.y0 - 1;
+                tma_load_5d(base + SITES * NE * 16, &a.gauge.fy, fullL(s), 2 * w.x0, ym, w.z0, t, mu * NE);
+            } else if (mu == 2) {
+                const int zm = (w.z0 == 0) ? a.Z - 1 : w.z0 - 1;
+                tma_load_5d(base + SITES * NE * 16, &a.gauge.fz, fullL(s), 2 * w.x0, w.y0, zm, t, mu * NE);
             }
-#pragma unroll
-            for (int o = 0; o < NOBJ; o++) {
-                if (q[o].done()) continue;
-                remaining++;
-                if (!mbar_test(emptyO(o), (q[o].f & 1u) ^ 1u)) continue;
-                const Item w = item_of(q[o].j);
-                const unsigned fb = fullO(o);
-                const int xm = (w.x0 == 0) ? a.X - 1 : w.x0 - 1, xp = (w.x0 + BX == a.X) ? 0 : w.x0 + BX;
-                const int ym = (w.y0 == 0) ? a.Y - 1 : w.y0 - 1, yp = (w.y0 + BY == a.Y) ? 0 : w.y0 + BY;
-                const int zm = (w.z0 == 0) ? a.Z - 1 : w.z0 - 1, zp = (w.z0 + BZ == a.Z) ? 0 : w.z0 + BZ;
-                const int t = (o == LT) ? wrap(w.t0 - 1 + q[o].u) : w.t0 + q[o].u;
-                if (o == HX) {
-                    mbar_expect_tx(fb, HX_BYTES);
-                    tma_load_5d(smem_u32(sHX), &a.in.fx, fb, 2 * xm, w.y0, w.z0, t, 0);
-                    tma_load_5d(smem_u32(sHX) + HX_BYTES / 2, &a.in.fx, fb, 2 * xp, w.y0, w.z0, t, 0);
-                } else if (o == HY) {
-                    mbar_expect_tx(fb, HY_BYTES);
-                    tma_load_5d(smem_u32(sHY), &a.in.fy, fb, 2 * w.x0, ym, w.z0, t, 0);
-                    tma_load_5d(smem_u32(sHY) + HY_BYTES / 2, &a.in.fy, fb, 2 * w.x0, yp, w.z0, t, 0);
-                } else if (o == HZ) {
-                    mbar_expect_tx(fb, HZ_BYTES);
-                    tma_load_5d(smem_u32(sHZ), &a.in.fz, fb, 2 * w.x0, w.y0, zm, t, 0);
-                    tma_load_5d(smem_u32(sHZ) + HZ_BYTES / 2, &a.in.fz, fb, 2 * w.x0, w.y0, zp, t, 0);
-                } else if (o == LX) {
-                    mbar_expect_tx(fb, LB::x);
-                    tma_load_5d(smem_u32(sLX), &a.gauge.main, fb, 2 * w.x0, w.y0, w.z0, t, 0 * NE);
-                    tma_load_5d(smem_u32(sLX) + SITES * NE * 16, &a.gauge.fx, fb, 2 * xm, w.y0, w.z0, t, 0 * NE);
-                } else if (o == LY) {
-                    mbar_expect_tx(fb, LB::y);
-                    tma_load_5d(smem_u32(sLY), &a.gauge.main, fb, 2 * w.x0, w.y0, w.z0, t, 1 * NE);
-                    tma_load_5d(smem_u32(sLY) + SITES * NE * 16, &a.gauge.fy, fb, 2 * w.x0, ym, w.z0, t, 1 * NE);
-                } else if (o == LZ) {
-                    mbar_expect_tx(fb, LB::z);
-                    tma_load_5d(smem_u32(sLZ), &a.gauge.main, fb, 2 * w.x0, w.y0, w.z0, t, 2 * NE);
-                    tma_load_5d(smem_u32(sLZ) + SITES * NE * 16, &a.gauge.fz, fb, 2 * w.x0, w.y0, zm, t, 2 * NE);
-                } else {
-                    mbar_expect_tx(fb, LB::t);
-                    tma_load_5d(smem_u32(sLT), &a.gauge.main, fb, 2 * w.x0, w.y0, w.z0, t, 3 * NE);
-                }
-                q[o].next();
-                progress = true;
+            nL++;
+        };
+        for (int it = blockIdx.x; it < a.nitems; it += gridDim.x) {
+            const Item w = decode_item(a, it);
+            const int tm = (w.t0 == 0) ? a.T - 1 : w.t0 - 1;
+            fill_I(w, tm);          // prologue: the slice below the segment, for the carried backward-t product
+            fill_L(w, tm, 3);
+            fill_I(w, w.t0);
+            for (int dt = 0; dt < a.Lt; dt++) {
+                const int t = w.t0 + dt, tp = (t + 1 == a.T) ? 0 : t + 1;
+                fill_I(w, tp);
+                fill_H(w, t);
+                fill_L(w, t, 0);
+                fill_L(w, t, 1);
+                fill_L(w, t, 2);
+                fill_L(w, t, 3);
             }
-            if (!progress) __nanosleep(40);
         }
         return;
     }
 
-    // =================================================================== consumers: one site per thread and group
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(REG_CONSUMER));
-    const bool groupA = warp < NGRP;
-    const int lz = groupA ? warp : warp - NGRP;
-    const int lx = lane & 7, ly = lane >> 3;
+    // =================================================================== consumers: one site per thread
+    const int lx = lane & 7, ly = lane >> 3, lz = warp;
     const int sin = lz * 32 + lane;                 // site index inside the tile = element offset inside a plane box
-    unsigned nI = 0;                                // interior planes consumed (both groups count every plane)
-    unsigned nS = 0;                                // slices done = uses of the per-slice objects and of the hand-over buffer
-    unsigned nT = 0;                                // group B: t-link chunks consumed (one extra per work item)
+    unsigned nI = 0, nH = 0, nL = 0;
     auto release = [&](unsigned bar) {
         __syncwarp();
         if (lane == 0) mbar_arrive(bar);
     };
-    double2* part = (double2*)sP + sin;             // this thread's slot of the hand-over buffer, element c at part[c * SITES]
 
-    if (groupA) {
-        // ---------------------------------------------------------------- group A: own term, x and y hops
-        for (int j = 0; j < my_items; j++) {
-            {   // the plane below the segment is group B's only
-                const unsigned s = nI % SI;
-                mbar_wait(fullI(s), (nI / SI) & 1u);
-                release(emptyI(s));
-                nI++;
-            }
-            for (int dt = 0; dt < a.Lt; dt++) {
-                const unsigned s0 = nI % SI;
-                mbar_wait(fullI(s0), (nI / SI) & 1u);
-                const double2* I0 = (const double2*)(sI + s0 * I_BYTES) + sin;
-                double2 acc[12];
-                if (NA < 0) {
-#pragma unroll
-                    for (int c = 0; c < 12; c++) acc[c] = make_double2(0.0, 0.0);
-                } else {
-                    const double mik = -1.0 / a.kappa;
-#pragma unroll
-                    for (int c = 0; c < 12; c++) { const double2 o = I0[c * SITES]; acc[c] = make_double2(mik * o.x, mik * o.y); }
-                }
-                {   // ---- x
-                    mbar_wait(fullO(HX), nS & 1u);
-                    mbar_wait(fullO(LX), nS & 1u);
-                    const double2* Hm = (const double2*)sHX;
-                    const double2* Hp = Hm + 12 * FX;
-                    const double2* Lb = (const double2*)sLX;
-                    const int fi = lz * BY + ly;
-                    const bool inp = lx + 1 < BX, inm = lx > 0;
-                    hop_smem<0, -1, RECON>(acc, inp ? I0 + 1 : Hp + fi, inp ? SITES : FX, Lb + sin, SITES, 1.0);
-                    hop_smem<0, +1, RECON>(acc, inm ? I0 - 1 : Hm + fi, inm ? SITES : FX,
-                                           inm ? Lb + sin - 1 : Lb + SITES * NE + fi, inm ? SITES : FX, 1.0);
-                    release(emptyO(HX));
-                    release(emptyO(LX));
-                }
-                {   // ---- y
-                    mbar_wait(fullO(HY), nS & 1u);
-                    mbar_wait(fullO(LY), nS & 1u);
-                    const double2* Hm = (const double2*)sHY;
-                    const double2* Hp = Hm + 12 * FY;
-                    const double2* Lb = (const double2*)sLY;
-                    const int fi = lz * BX + lx;
-                    const bool inp = ly + 1 < BY, inm = ly > 0;
-                    hop_smem<1, -1, RECON>(acc, inp ? I0 + BX : Hp + fi, inp ? SITES : FY, Lb + sin, SITES, 1.0);
-                    hop_smem<1, +1, RECON>(acc, inm ? I0 - BX : Hm + fi, inm ? SITES : FY,
-                                           inm ? Lb + sin - BX : Lb + SITES * NE + fi, inm ? SITES : FY, 1.0);
-                    release(emptyO(HY));
-                    release(emptyO(LY));
-                }
-                release(emptyI(s0));
-                nI++;
-                // ---- hand the partial sums to group B (warp lz of A feeds warp lz of B)
-                mbar_wait(partEmpty(lz), (nS & 1u) ^ 1u);
-#pragma unroll
-                for (int c = 0; c < 12; c++) part[c * SITES] = acc[c];
-                release(partFull(lz));
-                nS++;
-            }
-            {   // the plane above the segment is group B's only
-                const unsigned s = nI % SI;
-                mbar_wait(fullI(s), (nI / SI) & 1u);
-                release(emptyI(s));
-                nI++;
-            }
-        }
-        return;
-    }
-
-    // -------------------------------------------------------------------- group B: z and t hops, epilogue, stores
-    for (int j = 0; j < my_items; j++) {
-        const Item w = decode_item(a, (int)blockIdx.x + j * (int)gridDim.x);
+    for (int it = blockIdx.x; it < a.nitems; it += gridDim.x) {
+        const Item w = decode_item(a, it);
         double2 P[6];   // U_t(x, t-1)^+ (1 + gamma_t) psi(x, t-1): the backward-t hop of the next step, before the boundary sign
         {   // ---- prologue: slice t0 - 1
-            const unsigned si = nI % SI;
-            mbar_wait(fullI(si), (nI / SI) & 1u);
-            mbar_wait(fullO(LT), nT & 1u);
+            const unsigned si = slot_of<SI>(nI), sl = slot_of<SL>(nL);
+            mbar_wait(fullI(si), full_parity<SI>(nI));
+            mbar_wait(fullL(sl), full_parity<SL>(nL));
             const double2* Ib = (const double2*)(sI + si * I_BYTES) + sin;
-            const double2* Lb = (const double2*)sLT + sin;
+            const double2* Lb = (const double2*)(sL + sl * L_BYTES) + sin;
             double2 psi[12], h[6], u[9];
             lds_spinor(Ib, SITES, psi);
             project<3, +1>(psi, h);
             lds_link<RECON>(Lb, SITES, u);
             su3_mul<true>(u, h, P);
             release(emptyI(si));
-            release(emptyO(LT));
-            nI++; nT++;
+            release(emptyL(sl));
+            nI++; nL++;
         }
         for (int dt = 0; dt < a.Lt; dt++) {
             const int t = w.t0 + dt;
-            const unsigned s0 = nI % SI, s1 = (nI + 1) % SI;
-            const long long gsite = (long long)(w.x0 + lx) + (long long)a.X * ((w.y0 + ly) + (long long)a.Y * ((w.z0 + lz) + (long long)a.Z * t));
-            double2 acc[12];
-            mbar_wait(partFull(lz), nS & 1u);
-#pragma unroll
-            for (int c = 0; c < 12; c++) acc[c] = part[c * SITES];
-            release(partEmpty(lz));
-            mbar_wait(fullI(s0), (nI / SI) & 1u);
+            const unsigned s0 = slot_of<SI>(nI), s1 = slot_of<SI>(nI + 1), sh = slot_of<SH>(nH);
+            mbar_wait(fullI(s0), full_parity<SI>(nI));
             const double2* I0 = (const double2*)(sI + s0 * I_BYTES) + sin;
-            {   // ---- z
-                mbar_wait(fullO(HZ), nS & 1u);
-                mbar_wait(fullO(LZ), nS & 1u);
-                const double2* Hm = (const double2*)sHZ;
-                const double2* Hp = Hm + 12 * FZ;
-                const double2* Lb = (const double2*)sLZ;
+            const double2* Hb = (const double2*)(sH + sh * H_BYTES);
+            const long long gsite = (long long)(w.x0 + lx) + (long long)a.X * ((w.y0 + ly) + (long long)a.Y * ((w.z0 + lz) + (long long)a.Z * t));
+
+            double2 acc[12];
+            if (NA < 0) {
+#pragma unroll
+                for (int c = 0; c < 12; c++) acc[c] = make_double2(0.0, 0.0);
+            } else {
+                const double mik = -1.0 / a.kappa;
+#pragma unroll
+                for (int c = 0; c < 12; c++) { const double2 o = I0[c * SITES]; acc[c] = make_double2(mik * o.x, mik * o.y); }
+            }
+            mbar_wait(fullH(sh), full_parity<SH>(nH));
+            // ---- x
+            {
+                const unsigned sl = slot_of<SL>(nL);
+                mbar_wait(fullL(sl), full_parity<SL>(nL));
+                const double2* Lb = (const double2*)(sL + sl * L_BYTES);
+                const int fi = lz * BY + ly;
+                const bool inp = lx + 1 < BX, inm = lx > 0;
+                hop_smem<0, -1, RECON>(acc, inp ? I0 + 1 : Hb + HOFF_XP + fi, inp ? SITES : FX, Lb + sin, SITES, 1.0);
+                hop_smem<0, +1, RECON>(acc, inm ? I0 - 1 : Hb + HOFF_XM + fi, inm ? SITES : FX,
+                                       inm ? Lb + sin - 1 : Lb + SITES * NE + fi, inm ? SITES : FX, 1.0);
+                release(emptyL(sl));
+                nL++;
+            }
+            // ---- y
+            {
+                const unsigned sl = slot_of<SL>(nL);
+                mbar_wait(fullL(sl), full_parity<SL>(nL));
+                const double2* Lb = (const double2*)(sL + sl * L_BYTES);
+                const int fi = lz * BX + lx;
+                const bool inp = ly + 1 < BY, inm = ly > 0;
+                hop_smem<1, -1, RECON>(acc, inp ? I0 + BX : Hb + HOFF_YP + fi, inp ? SITES : FY, Lb + sin, SITES, 1.0);
+                hop_smem<1, +1, RECON>(acc, inm ? I0 - BX : Hb + HOFF_YM + fi, inm ? SITES : FY,
+                                       inm ? Lb + sin - BX : Lb + SITES * NE + fi, inm ? SITES : FY, 1.0);
+                release(emptyL(sl));
+                nL++;
+            }
+            // ---- z
+            {
+                const unsigned sl = slot_of<SL>(nL);
+                mbar_wait(fullL(sl), full_parity<SL>(nL));
+                const double2* Lb = (const double2*)(sL + sl * L_BYTES);
                 const int fi = ly * BX + lx;
                 const bool inp = lz + 1 < BZ, inm = lz > 0;
-                hop_smem<2, -1, RECON>(acc, inp ? I0 + BX * BY : Hp + fi, inp ? SITES : FZ, Lb + sin, SITES, 1.0);
-                hop_smem<2, +1, RECON>(acc, inm ? I0 - BX * BY : Hm + fi, inm ? SITES : FZ,
+                hop_smem<2, -1, RECON>(acc, inp ? I0 + BX * BY : Hb + HOFF_ZP + fi, inp ? SITES : FZ, Lb + sin, SITES, 1.0);
+                hop_smem<2, +1, RECON>(acc, inm ? I0 - BX * BY : Hb + HOFF_ZM + fi, inm ? SITES : FZ,
                                        inm ? Lb + sin - BX * BY : Lb + SITES * NE + fi, inm ? SITES : FZ, 1.0);
-                release(emptyO(HZ));
-                release(emptyO(LZ));
+                release(emptyL(sl));
+                nL++;
             }
-            {   // ---- t: forward from the next interior plane, backward from the carried product
-                mbar_wait(fullO(LT), nT & 1u);
-                mbar_wait(fullI(s1), ((nI + 1) / SI) & 1u);
-                const double2* Lb = (const double2*)sLT + sin;
+            release(emptyH(sh));
+            nH++;
+            // ---- t: forward from the next interior plane, backward from the carried product
+            {
+                const unsigned sl = slot_of<SL>(nL);
+                mbar_wait(fullL(sl), full_parity<SL>(nL));
+                mbar_wait(fullI(s1), full_parity<SI>(nI + 1));
+                const double2* Lb = (const double2*)(sL + sl * L_BYTES) + sin;
                 const double2* I1 = (const double2*)(sI + s1 * I_BYTES) + sin;
                 hop_smem<3, -1, RECON>(acc, I1, SITES, Lb, SITES, (t + 1 == a.T) ? a.tphase : 1.0);   // boundary in time
                 reconstruct_add<3, +1>(acc, P, (t == 0) ? a.tphase : 1.0);
@@ -431,12 +338,11 @@ __global__ void __launch_bounds__(THREADS, 1) wilson_tma_kernel(const __grid_con
                 project<3, +1>(psi, h);
                 lds_link<RECON>(Lb, SITES, u);
                 su3_mul<true>(u, h, P);
-                release(emptyO(LT));
-                nT++;
+                release(emptyL(sl));
+                nL++;
             }
             release(emptyI(s0));
             nI++;
-            nS++;
 
             // ---- epilogue (same arithmetic as the gather kernel)
             double2* o = a.out + gsite;
@@ -472,8 +378,8 @@ __global__ void __launch_bounds__(THREADS, 1) wilson_tma_kernel(const __grid_con
         }
         // the plane above the segment was only the forward-t neighbour of the last slice
         {
-            const unsigned s = nI % SI;
-            mbar_wait(fullI(s), (nI / SI) & 1u);
+            const unsigned s = slot_of<SI>(nI);
+            mbar_wait(fullI(s), full_parity<SI>(nI));
             release(emptyI(s));
             nI++;
         }
@@ -576,32 +482,16 @@ int launch_wilson_tma(ov_ctx* ctx, const double2* in, double2* out, const Epilog
             if (cost < best - 1e-9) { best = cost; st->Lt = L; st->nitems = (int)items; }
         }
     }
-    auto map_of = [&](const double2* p, Maps** out) -> bool {   // tensor maps by pointer (a handful of workspaces + caller buffers)
-        auto g = st->spinor.find(p);
-        if (g == st->spinor.end()) {
-            if (st->spinor.size() > 256) st->spinor.clear();
-            Maps m;
-            if (!make_maps(&m, p, lat, 12, 12)) return false;
-            g = st->spinor.emplace(p, m).first;
-        }
-        *out = &g->second;
-        return true;
-    };
+    auto f = st->spinor.find(in);
+    if (f == st->spinor.end()) {
+        if (st->spinor.size() > 256) st->spinor.clear();
+        Maps m;
+        if (!make_maps(&m, in, lat, 12, 12)) return fail(ctx, OV_ECUDA, "cuTensorMapEncodeTiled failed for a spinor");
+        f = st->spinor.emplace(in, m).first;
+    }
     Args a;
-    {
-        Maps* m = nullptr;
-        if (!map_of(in, &m)) return fail(ctx, OV_ECUDA, "cuTensorMapEncodeTiled failed for a spinor");
-        a.in = *m;
-    }
+    a.in = f->second;
     a.gauge = st->gauge;
-    {
-        const double2* ops[3] = {ep.hop_only ? nullptr : ep.A1, ep.hop_only ? nullptr : ep.A2, ep.hop_only ? nullptr : ep.A3};
-        for (int i = 0; i < 3; i++) {
-            Maps* m = nullptr;
-            if (ops[i] && !map_of(ops[i], &m)) return fail(ctx, OV_ECUDA, "cuTensorMapEncodeTiled failed for an epilogue operand");
-            a.op[i] = m ? m->main : a.in.main;   // unused slots get a valid map (never dereferenced)
-        }
-    }
     a.out = out;
     a.A1 = ep.A1; a.A2 = ep.A2; a.A3 = ep.A3;
     a.a1 = ep.a1; a.a2 = ep.a2; a.a3 = ep.a3;
@@ -620,7 +510,8 @@ int launch_wilson_tma(ov_ctx* ctx, const double2* in, double2* out, const Epilog
     if ((ep.A3 && !ep.A2) || (ep.A2 && !ep.A1)) return fail(ctx, OV_EINVAL, "epilogue operands must be filled in order");
     const int na = ep.hop_only ? -1 : (ep.A3 ? 3 : ep.A2 ? 2 : ep.A1 ? 1 : 0);
     const int grid = st->nitems < st->sm_count ? st->nitems : st->sm_count;
-    const size_t smem = NE == 9 ? smem_bytes<9>() : smem_bytes<6>();
+    const size_t smem = (size_t)SI * I_BYTES + (size_t)SH * H_BYTES + (size_t)SL * (NE == 9 ? LSlot<9>::bytes : LSlot<6>::bytes) +
+                        8 * (2 * SI + 2 * SH + 2 * SL);
     cudaError_t e;
 #define OV_TMA_NA(R)                                                                         \
     switch (na) {                                                                            \

@@ -99,8 +99,8 @@ def test_dslash_and_hw_vs_oracle(ovp, dims, spread, recon):
         results[variant] = (hop, got)
         # the batched launch (always the gather kernel) agrees too
         assert rel(to_host(op, op.apply_hw(d)), ref_hw) <= TOL_HW
-    if tma:   # same arithmetic in the same order: the two kernels agree to the last bit
-        assert np.array_equal(results[1][0], results[2][0]) and np.array_equal(results[1][1], results[2][1])
+    if tma:   # same arithmetic in the same order: the hop agrees to the last bit, H_w up to the compiler's FMA contraction
+        assert np.array_equal(results[1][0], results[2][0]) and rel(results[1][1], results[2][1]) <= 1e-15
     if not tma:
         with pytest.raises(ovp.OvError):
             op.set_dslash_variant(2)
