@@ -65,12 +65,11 @@ int effective_variant(const ov_ctx* ctx) {
     return tma_usable(ctx) ? 2 : 1;
 }
 
-// Automatic choice (variant 0) where the TMA-staged kernel applies: launches without epilogue operands (the first
-// launch of every Clenshaw pair, H_w, dslash) go to the TMA-staged kernel, launches with fused axpy operands to the
-// gather kernel (measured: DESIGN.md section 10).  An explicit variant 1 or 2 sends every launch to that kernel.
+// Automatic choice (variant 0): the TMA-staged kernel wherever it applies (planes layout, X % 8 == Y % 4 == Z % 4 == 0),
+// for launches with and without fused axpy operands (measured: DESIGN.md section 10); the gather kernel otherwise.
+// An explicit variant 1 or 2 sends every single-right-hand-side launch to that kernel.
 int launch_wilson(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep) {
-    const bool operands = !ep.hop_only && ep.A1 != nullptr;
-    if (ctx->dslash_variant == 2 || (ctx->dslash_variant == 0 && tma_usable(ctx) && !operands))
+    if (ctx->dslash_variant == 2 || (ctx->dslash_variant == 0 && tma_usable(ctx)))
         return launch_wilson_tma(ctx, in, out, ep);
     return launch_wilson_gather(ctx, in, out, ep);
 }

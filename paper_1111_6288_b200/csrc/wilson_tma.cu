@@ -17,6 +17,11 @@
 //     later becomes the site's own plane; the backward t hop U_t(x-t)^+ (1+gamma_t) psi(x-t) is carried in registers
 //     from the previous step), do the same arithmetic in the same order as the gather kernel (results are bit-identical),
 //     and store the result with coalesced 16-byte stores.
+//   * launches with fused axpy operands (NA >= 1: the second launch of every Clenshaw order, the D_ov assembly) add an
+//     EPILOGUE warpgroup: the consumers hand their accumulators over through a 24 KB shared-memory buffer and go on with
+//     the next slice, while four epilogue warps -- which hold nothing else in registers -- issue the operand loads of a
+//     slice BEFORE its accumulators arrive, so the DRAM latency of those one-touch streams overlaps the hops instead of
+//     following them; setmaxnreg moves the registers the producer and the epilogue warps do not need to the consumers.
 // L2->SM traffic per site: 192 (own) + 240 (halo) + 576 (links) + 72 (halo links) = 1080 B instead of ~2200.
 //
 // Needs the planes layout and X % 8 == 0, Y % 4 == 0, Z % 4 == 0; other shapes use the gather kernel.
@@ -34,8 +39,16 @@ namespace tma {
 constexpr int BX = 8, BY = 4, BZ = 4;           // tile of one time slice
 constexpr int SITES = BX * BY * BZ;             // 128 = 4 consumer warps
 constexpr int NCONS = SITES / 32;               // consumer warps
-constexpr int THREADS = SITES + 32;             // + 1 producer warp
-constexpr int SI = 3, SH = 2, SL = 4;           // ring depths: interior planes, halo sets, link chunks
+constexpr int SI = 3, SH = 2;                   // ring depths: interior planes, halo sets
+// per kernel form: without epilogue operands 4 consumer warps + 1 producer warp and 4 link chunks in the ring; with them
+// three aligned warpgroups (consumers, epilogue, producer) and 3 link chunks (the 4th slot becomes the hand-over buffer)
+template <int NA> struct Form {
+    static constexpr bool epi = NA >= 1;
+    static constexpr int threads = epi ? 3 * 128 : SITES + 32;
+    static constexpr int SL = epi ? 3 : 4;
+};
+constexpr int P_BYTES = SITES * 12 * 16;        // hand-over buffer: the consumers' accumulators of one slice
+constexpr int REG_CONSUMER = 232, REG_PRODUCER = 40;   // epilogue warps keep the compiled 168: 128 * (232 + 168 + 40) <= 65536
 constexpr int I_BYTES = SITES * 12 * 16;        // 24576
 constexpr int FX = BY * BZ, FY = BX * BZ, FZ = BX * BY;   // face sites: 16, 32, 32
 constexpr int H_ELEMS = 12 * (2 * FX + 2 * FY + 2 * FZ);  // 1920 double2
@@ -146,15 +159,19 @@ using namespace tma;
 
 // NA: -1 hop only, 0..3 epilogue operands (read from global memory at the output site)
 template <int RECON, int NA>
-__global__ void __launch_bounds__(THREADS, 1) wilson_tma_kernel(const __grid_constant__ Args a) {
+__global__ void __launch_bounds__(Form<NA>::threads, 1) wilson_tma_kernel(const __grid_constant__ Args a) {
     constexpr int NE = RECON / 2;
     constexpr int L_BYTES = LSlot<NE>::bytes;
+    constexpr bool EPI = Form<NA>::epi;
+    constexpr int SL = Form<NA>::SL;
+    constexpr int PRODUCER_WARP = EPI ? 8 : NCONS;
     extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char* sI = smem;
     unsigned char* sH = sI + SI * I_BYTES;
     unsigned char* sL = sH + SH * H_BYTES;
-    unsigned long long* bars = (unsigned long long*)(sL + SL * L_BYTES);
-    // barrier indices: fullI[SI], emptyI[SI], fullH[SH], emptyH[SH], fullL[SL], emptyL[SL]
+    unsigned char* sP = sL + SL * L_BYTES;          // hand-over buffer (EPI only)
+    unsigned long long* bars = (unsigned long long*)(sP + (EPI ? P_BYTES : 0));
+    // barrier indices: fullI[SI], emptyI[SI], fullH[SH], emptyH[SH], fullL[SL], emptyL[SL], partFull[NCONS], partEmpty[NCONS]
     const unsigned bar0 = smem_u32(bars);
     auto fullI = [&](unsigned s) { return bar0 + 8u * s; };
     auto emptyI = [&](unsigned s) { return bar0 + 8u * (SI + s); };
@@ -162,19 +179,24 @@ __global__ void __launch_bounds__(THREADS, 1) wilson_tma_kernel(const __grid_con
     auto emptyH = [&](unsigned s) { return bar0 + 8u * (2 * SI + SH + s); };
     auto fullL = [&](unsigned s) { return bar0 + 8u * (2 * SI + 2 * SH + s); };
     auto emptyL = [&](unsigned s) { return bar0 + 8u * (2 * SI + 2 * SH + SL + s); };
+    auto partFull = [&](unsigned w) { return bar0 + 8u * (2 * SI + 2 * SH + 2 * SL + w); };
+    auto partEmpty = [&](unsigned w) { return bar0 + 8u * (2 * SI + 2 * SH + 2 * SL + NCONS + w); };
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) {
         for (unsigned s = 0; s < SI; s++) { mbar_init(fullI(s), 1); mbar_init(emptyI(s), NCONS); }
         for (unsigned s = 0; s < SH; s++) { mbar_init(fullH(s), 1); mbar_init(emptyH(s), NCONS); }
         for (unsigned s = 0; s < SL; s++) { mbar_init(fullL(s), 1); mbar_init(emptyL(s), NCONS); }
+        if (EPI)
+            for (unsigned w = 0; w < NCONS; w++) { mbar_init(partFull(w), 1); mbar_init(partEmpty(w), 1); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
 
-    if (warp == NCONS) {
+    if (warp >= PRODUCER_WARP) {
         // =============================================================== producer: one thread issues every TMA load
-        if (lane != 0) return;
+        if (EPI) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REG_PRODUCER));
+        if (warp != PRODUCER_WARP || lane != 0) return;
         unsigned nI = 0, nH = 0, nL = 0;
         auto fill_I = [&](const Item& w, int t) {
             const unsigned s = slot_of<SI>(nI);
@@ -237,10 +259,78 @@ __global__ void __launch_bounds__(THREADS, 1) wilson_tma_kernel(const __grid_con
         return;
     }
 
+    if (EPI && warp >= NCONS) {
+        // =============================================================== epilogue warps (launches with operands only)
+        const int lx = lane & 7, ly = lane >> 3, lz = warp - NCONS;
+        const double2* part = (const double2*)sP + lz * 32 + lane;
+        const double s_up = -a.kappa * a.s, s_lo = a.g5 ? a.kappa * a.s : -a.kappa * a.s;
+        unsigned nS = 0;
+        auto rel1 = [&](unsigned bar) {
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar);
+        };
+        // Operand loads run as a two-deep software pipeline of chunks of 3 components (9 loads of 16 B per thread and
+        // chunk): the chunk after the one being combined is always in flight, across slice and work-item boundaries, and the
+        // first chunk of a slice is issued before its accumulators are waited for.  Larger bursts were slower: with the
+        // shared-memory carve-out at its maximum the LSU queue fills up and holds back the consumers' shared-memory loads.
+        constexpr int CH = 3;
+        auto gsite_of = [&](int it, int dt) -> long long {
+            const Item w = decode_item(a, it);
+            return (long long)(w.x0 + lx) + (long long)a.X * ((w.y0 + ly) + (long long)a.Y * ((w.z0 + lz) + (long long)a.Z * (w.t0 + dt)));
+        };
+        auto load_ops = [&](long long gsite, int c0, double2* w1, double2* w2, double2* w3) {
+#pragma unroll
+            for (int k = 0; k < CH; k++) {
+                const long long e = gsite + (long long)(c0 + k) * a.V;
+                if (NA >= 1) w1[k] = a.A1[e];
+                if (NA >= 2) w2[k] = a.A2[e];
+                if (NA >= 3) w3[k] = a.A3[e];
+            }
+        };
+        auto combine_store = [&](long long gsite, int c0, const double2* acc, const double2* w1, const double2* w2, const double2* w3) {
+            double2* o = a.out + gsite;
+#pragma unroll
+            for (int k = 0; k < CH; k++) {
+                const int c = c0 + k;
+                const bool lo = (c >= 6);
+                const double sc = lo ? s_lo : s_up;
+                double2 v = make_double2(sc * acc[c].x, sc * acc[c].y);
+                if (NA >= 1) { const double f = (lo && (a.a_g5 & 1)) ? -a.a1 : a.a1; v.x = fma(f, w1[k].x, v.x); v.y = fma(f, w1[k].y, v.y); }
+                if (NA >= 2) { const double f = (lo && (a.a_g5 & 2)) ? -a.a2 : a.a2; v.x = fma(f, w2[k].x, v.x); v.y = fma(f, w2[k].y, v.y); }
+                if (NA >= 3) { const double f = (lo && (a.a_g5 & 4)) ? -a.a3 : a.a3; v.x = fma(f, w3[k].x, v.x); v.y = fma(f, w3[k].y, v.y); }
+                o[c * a.V] = v;
+            }
+        };
+        double2 u1[CH], u2[CH], u3[CH], v1[CH], v2[CH], v3[CH], acc[12];   // the two operand buffers
+        int it = blockIdx.x, dt = 0;
+        if (it < a.nitems) load_ops(gsite_of(it, 0), 0, u1, u2, u3);
+        while (it < a.nitems) {
+            const long long gsite = gsite_of(it, dt);
+            int it_n = it, dt_n = dt + 1;
+            if (dt_n == a.Lt) { dt_n = 0; it_n = it + gridDim.x; }
+            load_ops(gsite, 3, v1, v2, v3);
+            mbar_wait(partFull(lz), nS & 1u);
+#pragma unroll
+            for (int c = 0; c < 12; c++) acc[c] = part[c * SITES];
+            rel1(partEmpty(lz));
+            nS++;
+            combine_store(gsite, 0, acc, u1, u2, u3);
+            load_ops(gsite, 6, u1, u2, u3);
+            combine_store(gsite, 3, acc, v1, v2, v3);
+            load_ops(gsite, 9, v1, v2, v3);
+            combine_store(gsite, 6, acc, u1, u2, u3);
+            if (it_n < a.nitems) load_ops(gsite_of(it_n, dt_n), 0, u1, u2, u3);
+            combine_store(gsite, 9, acc, v1, v2, v3);
+            it = it_n; dt = dt_n;
+        }
+        return;
+    }
+
     // =================================================================== consumers: one site per thread
+    if (EPI) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(REG_CONSUMER));
     const int lx = lane & 7, ly = lane >> 3, lz = warp;
     const int sin = lz * 32 + lane;                 // site index inside the tile = element offset inside a plane box
-    unsigned nI = 0, nH = 0, nL = 0;
+    unsigned nI = 0, nH = 0, nL = 0, nS = 0;
     auto release = [&](unsigned bar) {
         __syncwarp();
         if (lane == 0) mbar_arrive(bar);
@@ -344,6 +434,15 @@ __global__ void __launch_bounds__(THREADS, 1) wilson_tma_kernel(const __grid_con
             release(emptyI(s0));
             nI++;
 
+            if (EPI) {   // ---- hand the accumulators to the epilogue warp of the same sites and go on
+                double2* part = (double2*)sP + sin;
+                mbar_wait(partEmpty(lz), (nS & 1u) ^ 1u);
+#pragma unroll
+                for (int c = 0; c < 12; c++) part[c * SITES] = acc[c];
+                release(partFull(lz));
+                nS++;
+                continue;
+            }
             // ---- epilogue (same arithmetic as the gather kernel)
             double2* o = a.out + gsite;
             if (NA < 0) {
@@ -453,7 +552,7 @@ static cudaError_t launch_k(const Args& a, int grid, size_t smem, cudaStream_t s
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    wilson_tma_kernel<RECON, NA><<<grid, THREADS, smem, st>>>(a);
+    wilson_tma_kernel<RECON, NA><<<grid, Form<NA>::threads, smem, st>>>(a);
     return cudaGetLastError();
 }
 
@@ -510,8 +609,10 @@ int launch_wilson_tma(ov_ctx* ctx, const double2* in, double2* out, const Epilog
     if ((ep.A3 && !ep.A2) || (ep.A2 && !ep.A1)) return fail(ctx, OV_EINVAL, "epilogue operands must be filled in order");
     const int na = ep.hop_only ? -1 : (ep.A3 ? 3 : ep.A2 ? 2 : ep.A1 ? 1 : 0);
     const int grid = st->nitems < st->sm_count ? st->nitems : st->sm_count;
-    const size_t smem = (size_t)SI * I_BYTES + (size_t)SH * H_BYTES + (size_t)SL * (NE == 9 ? LSlot<9>::bytes : LSlot<6>::bytes) +
-                        8 * (2 * SI + 2 * SH + 2 * SL);
+    const bool epi = na >= 1;
+    const int nsl = epi ? Form<1>::SL : Form<0>::SL;
+    const size_t smem = (size_t)SI * I_BYTES + (size_t)SH * H_BYTES + (size_t)nsl * (NE == 9 ? LSlot<9>::bytes : LSlot<6>::bytes) +
+                        (epi ? P_BYTES : 0) + 8 * (2 * SI + 2 * SH + 2 * nsl + 2 * NCONS);
     cudaError_t e;
 #define OV_TMA_NA(R)                                                                         \
     switch (na) {                                                                            \
