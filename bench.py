@@ -53,6 +53,8 @@ def parse_args():
                     help="--impl reference: wall-clock budget for the measured oracle steps (counts are cut to fit)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cg", action="store_true")
+    ap.add_argument("--no-deflation", action="store_true",
+                    help="skip the deflated multi-mass CG extra (workloads.DEFLATION, 16^3x32 smooth links, ~1 min)")
     ap.add_argument("--kernels", action="store_true",
                     help="time every kernel class of the path alone (CUDA events) and print a per-kernel roofline table")
     ap.add_argument("--reps", type=int, default=0, help="with --kernels: launches per kernel class (0 = defaults)")
@@ -439,6 +441,10 @@ def run_b200(args):
                 cg[name]["orders"] = op.cg_orders()
         op.set_cg_adaptive(0)
         del xs, bsrc
+    # ---- deflated multi-mass CG on the workload built for it, reported separately
+    deflation = None
+    if world == 1 and not args.no_cg and not args.no_deflation and args.config == 3:
+        deflation = deflation_extra(ovp, log)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -452,7 +458,52 @@ def run_b200(args):
             Vh[i] = op.unpack_spinor(Vlow[i]).cpu().numpy()
         modes_host = (Vh, np.asarray(lam))
     return finish(args, cfg, order, k, V_sites, world, ms, value, launches, tim, e2e, hw_gbs, ms_hw / nhw,
-                  sampler, lanczos_s, resid, U, log, cg, batched, recon12, modes_host, op.dslash_variant)
+                  sampler, lanczos_s, resid, U, log, cg, batched, recon12, modes_host, op.dslash_variant, deflation)
+
+
+def deflation_extra(ovp, log):
+    """Low modes of D_ov (per chirality sector) + deflated multi-mass CG on workloads.DEFLATION: 16^3x32, smooth links,
+    periodic time (six near-zero modes of D_ov^+ D_ov per sector), 6 masses, point source, tol 1e-8."""
+    import torch
+    cfg = wl.DEFLATION
+    U = wl.su3_links(cfg.dims, cfg.spread, wl.gauge_seed(cfg.index))
+    op = ovp.Overlap(cfg.dims, cfg.kappa, U, t_boundary=wl.DEFLATION_T_BOUNDARY)
+    op.set_polynomial(ovp.chebyshev_coeffs(10, 0.01), 0.01, cfg.norm)
+    t0 = time.perf_counter()
+    V, lam, _, ok = op.lanczos_lowmodes(16, tol=1e-9, max_restarts=60, cheb_order=100)
+    se = 0.95 * float(np.max(np.abs(lam)))
+    n = int(np.ceil(np.log(0.41 / 1e-12) / (2.1 * se)))          # delta ~ 1e-12 (PAPER.md:37, eq. 2.2)
+    op.set_polynomial(ovp.chebyshev_coeffs(n, se * se), se * se, cfg.norm)
+    op.set_smallspace(V, lam)
+    t_hw = time.perf_counter() - t0
+    k = 12
+    t0 = time.perf_counter()
+    Ws, mus = [], []
+    for s in (+1, -1):
+        W, mu, res, ok2 = op.lanczos_dov_lowmodes(s, k, tol=1e-9, max_restarts=60, cheb_order=12)
+        ok = ok and ok2
+        Ws.append(W)
+        mus.append(mu)
+    torch.cuda.synchronize()
+    t_modes = time.perf_counter() - t0
+    b = op.pack_spinor(torch.from_numpy(wl.point_source(cfg.dims)).cuda())
+    out = {"workload": f"{cfg.name}, spread {cfg.spread}, Chebyshev order {n}, sqrt(eps) {se:.4f}, 16 H_w modes",
+           "masses": list(cfg.masses), "tol": 1e-8, "source": "point", "modes_per_sector": k, "dov_filter_order": 12,
+           "hw_modes_seconds": t_hw, "dov_modes_seconds": t_modes, "modes_converged": bool(ok),
+           "mu_min": float(min(m.min() for m in mus)), "mu_max": float(max(m.max() for m in mus))}
+    for name, defl in (("plain", False), ("deflated", True)):
+        op.set_deflation(torch.cat(Ws).contiguous() if defl else None, np.concatenate(mus) if defl else None)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        _, iters, relres, okc = op.multishift_cg(list(cfg.masses), b, tol=1e-8, maxiter=5000)
+        torch.cuda.synchronize()
+        out[name] = {"seconds": time.perf_counter() - t0, "iterations": iters, "converged": bool(okc),
+                     "max_true_residual": float(np.max(relres)), "note": "seconds include the true-residual check (12 D_ov applies)"}
+    op.set_deflation(None, None)
+    log(f"deflation extra: {out['plain']['iterations']} -> {out['deflated']['iterations']} iterations, "
+        f"{out['plain']['seconds']:.1f} -> {out['deflated']['seconds']:.1f} s, D_ov modes {t_modes:.0f} s")
+    op.close()
+    return out
 
 
 class _Null:
@@ -493,7 +544,7 @@ def ncu_traffic(config, recon, order, kernel):
 
 
 def finish(args, cfg, order, k, V_sites, world, ms, value, launches, tim, e2e, hw_gbs, hw_ms, sampler,
-           lanczos_s, resid, U, log, cg=None, batched=None, recon12=None, modes_host=None, variant_used=1):
+           lanczos_s, resid, U, log, cg=None, batched=None, recon12=None, modes_host=None, variant_used=1, deflation=None):
     peak, peak_src = measured_peak()
     nsign = args.steps
     wl_launches = tim["wilson_launches"]
@@ -529,7 +580,7 @@ def finish(args, cfg, order, k, V_sites, world, ms, value, launches, tim, e2e, h
                    "dslash_variant": variant_used, "layout": args.layout,
                    "l2": "inputs larger than L2 (gauge 510 MB + 17 GB of low modes stream every step)",
                    "low_modes": f"GPU Lanczos, max residual {resid:.1e}, {lanczos_s:.0f} s (untimed setup)" if k else "none"},
-        "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu, "cg_time_to_solution": cg, "batched": batched, "recon12": recon12,
+        "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu, "cg_time_to_solution": cg, "deflated_cg": deflation, "batched": batched, "recon12": recon12,
         "paper_context": "paper: ~30 CPU cores per GPU on unnamed 6 GB GPUs vs Cray XT-5 (PAPER.md:9) - context only",
     }
     print(json.dumps(line), flush=True)

@@ -179,6 +179,7 @@ void ov_destroy(ov_ctx* ctx) {
     if (ctx->h_result) cudaFreeHost(ctx->h_result);
     cudaFree(ctx->d_sgn);
     cudaFree(ctx->d_coef);
+    cudaFree(ctx->d_coefb);
     cudaFree(ctx->host_stage_in);
     cudaFree(ctx->host_stage_abi);
     cudaFree(ctx->host_stage_out);

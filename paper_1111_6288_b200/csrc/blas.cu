@@ -315,29 +315,37 @@ __device__ __forceinline__ void dot_load4(const double2* __restrict__ xs, size_t
         }
 }
 
+// NB right-hand sides y_r = y + r * ystride at once (the batched small-space projector, "adding a new source
+// is relatively inexpensive"): every x_j is still streamed ONCE, its window is reduced against the NB windows of y kept in
+// registers.  Results: partial[(r * nvec + j) * nblocks + block].
+template <int NB>
 __global__ void __launch_bounds__(kDotThreads) multi_dot_kernel(const double2* __restrict__ xs, size_t stride,
-                                                                int nvec, const double2* __restrict__ y,
+                                                                int nvec, const double2* __restrict__ y, size_t ystride,
                                                                 long long n, long long nblocks,
                                                                 double2* __restrict__ partial) {
-    extern __shared__ double2 sacc[];  // [nvec][kDotWarps]
+    extern __shared__ double2 sacc[];  // [NB][nvec][kDotWarps]
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const long long base = (long long)blockIdx.x * kDotBlockElems + warp * (kDotE * 32) + lane;
-    double2 yv[kDotE];
+    double2 yv[NB][kDotE];
 #pragma unroll
-    for (int m = 0; m < kDotE; m++) {
-        const long long e = base + m * 32;
-        yv[m] = (e < n) ? y[e] : make_double2(0.0, 0.0);
-    }
+    for (int r = 0; r < NB; r++)
+#pragma unroll
+        for (int m = 0; m < kDotE; m++) {
+            const long long e = base + m * 32;
+            yv[r][m] = (e < n) ? y[(size_t)r * ystride + e] : make_double2(0.0, 0.0);
+        }
     double2 cur[4][kDotE], nxt[4][kDotE];
     dot_load4(xs, stride, 0, nvec, base, n, cur);
     for (int j = 0; j < nvec; j += 4) {
         dot_load4(xs, stride, j + 4, nvec, base, n, nxt);   // next four in flight while these are reduced
+#pragma unroll
+      for (int r = 0; r < NB; r++) {
         double v[8];
 #pragma unroll
         for (int u = 0; u < 4; u++) {
             double2 acc = make_double2(0.0, 0.0);
 #pragma unroll
-            for (int m = 0; m < kDotE; m++) cmaddc(acc, cur[u][m], yv[m]);
+            for (int m = 0; m < kDotE; m++) cmaddc(acc, cur[u][m], yv[r][m]);
             v[2 * u] = acc.x; v[2 * u + 1] = acc.y;
         }
         // halving butterfly: 8 -> 4 -> 2 -> 1 values per lane, then two plain steps
@@ -364,15 +372,16 @@ __global__ void __launch_bounds__(kDotThreads) multi_dot_kernel(const double2* _
         if ((lane & 3) == 0) {
             const int idx = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
             const int jj = j + (idx >> 1);
-            if (jj < nvec) reinterpret_cast<double*>(sacc + (size_t)jj * kDotWarps + warp)[idx & 1] = v[0];
+            if (jj < nvec) reinterpret_cast<double*>(sacc + ((size_t)r * nvec + jj) * kDotWarps + warp)[idx & 1] = v[0];
         }
+      }
 #pragma unroll
         for (int u = 0; u < 4; u++)
 #pragma unroll
             for (int m = 0; m < kDotE; m++) cur[u][m] = nxt[u][m];
     }
     __syncthreads();
-    for (int jj = threadIdx.x; jj < nvec; jj += kDotThreads) {
+    for (int jj = threadIdx.x; jj < NB * nvec; jj += kDotThreads) {
         double2 t = sacc[(size_t)jj * kDotWarps];
 #pragma unroll
         for (int w = 1; w < kDotWarps; w++) t = cadd(t, sacc[(size_t)jj * kDotWarps + w]);
@@ -406,10 +415,10 @@ int launch_multi_dot_at(ov_ctx* ctx, const double2* xs, size_t stride, int nvec,
         const int nv = std::min(kDotMaxVec, nvec - j0);
         const size_t shmem = (size_t)nv * kDotWarps * sizeof(double2);
         if (shmem > 48 * 1024)
-            OV_CUDA(ctx, cudaFuncSetAttribute(multi_dot_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shmem));
+            OV_CUDA(ctx, cudaFuncSetAttribute(multi_dot_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shmem));
         double2* partial = ctx->d_partial + (size_t)(result_offset + j0) * nblocks;
-        multi_dot_kernel<<<(unsigned)nblocks, kDotThreads, shmem, ctx->stream>>>(xs + (size_t)j0 * stride, stride, nv, y, n,
-                                                                                  nblocks, partial);
+        multi_dot_kernel<1><<<(unsigned)nblocks, kDotThreads, shmem, ctx->stream>>>(xs + (size_t)j0 * stride, stride, nv, y, 0, n,
+                                                                                     nblocks, partial);
         reduce_partials_kernel<<<nv, kRedThreads, 0, ctx->stream>>>(partial, nblocks, ctx->d_result + result_offset + j0);
         ctx->launches += 2;
     }
@@ -419,6 +428,29 @@ int launch_multi_dot_at(ov_ctx* ctx, const double2* xs, size_t stride, int nvec,
 
 int launch_multi_dot(ov_ctx* ctx, const double2* xs, size_t stride, int nvec, const double2* y) {
     return launch_multi_dot_at(ctx, xs, stride, nvec, y, 0, nvec);
+}
+
+// nb in {2, 4} right-hand sides y_r = y + r * ystride in one pass over the x_j: d_result[r * nvec + j] = <x_j, y_r>
+int launch_multi_dot_batch(ov_ctx* ctx, const double2* xs, size_t stride, int nvec, const double2* y, size_t ystride, int nb) {
+    const long long n = (long long)spinor_elems(ctx);
+    const long long nblocks = (n + kDotBlockElems - 1) / kDotBlockElems;
+    if (nb != 2 && nb != 4) return fail(ctx, OV_EINVAL, "multi_dot_batch: nb must be 2 or 4");
+    const size_t shmem = (size_t)nb * nvec * kDotWarps * sizeof(double2);
+    if (shmem > 200 * 1024) return fail(ctx, OV_EINVAL, "multi_dot_batch: %d x %d results do not fit in shared memory", nb, nvec);
+    OV_TRY(ensure_reduction_buffers(ctx, (size_t)nblocks * nb * nvec, (size_t)nb * nvec));
+    if (nb == 2) {
+        if (shmem > 48 * 1024)
+            OV_CUDA(ctx, cudaFuncSetAttribute(multi_dot_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shmem));
+        multi_dot_kernel<2><<<(unsigned)nblocks, kDotThreads, shmem, ctx->stream>>>(xs, stride, nvec, y, ystride, n, nblocks, ctx->d_partial);
+    } else {
+        if (shmem > 48 * 1024)
+            OV_CUDA(ctx, cudaFuncSetAttribute(multi_dot_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shmem));
+        multi_dot_kernel<4><<<(unsigned)nblocks, kDotThreads, shmem, ctx->stream>>>(xs, stride, nvec, y, ystride, n, nblocks, ctx->d_partial);
+    }
+    reduce_partials_kernel<<<nb * nvec, kRedThreads, 0, ctx->stream>>>(ctx->d_partial, nblocks, ctx->d_result);
+    ctx->launches += 2;
+    OV_CUDA(ctx, cudaGetLastError());
+    return OV_OK;
 }
 
 int fetch_results(ov_ctx* ctx, int n, double2* host_out) {
@@ -489,7 +521,10 @@ __global__ void __launch_bounds__(kMaThreads) multi_axpy_kernel(const double2* _
     double2 acc[J];
     const double2 b = base ? base[e] : make_double2(0.0, 0.0);
 #pragma unroll
-    for (int j = 0; j < J; j++) acc[j] = make_double2(o.bscale[j] * b.x, o.bscale[j] * b.y);
+    for (int j = 0; j < J; j++) {
+        const double2 bj = o.basej[j] ? o.basej[j][e] : b;      // per-output base (batched projector) or the common one
+        acc[j] = make_double2(o.bscale[j] * bj.x, o.bscale[j] * bj.y);
+    }
     int i = 0;
     for (; i + 4 <= nvec; i += 4) {
         double2 xv[4];

@@ -89,6 +89,8 @@ struct ov_ctx {
     double* d_sgn = nullptr;       // k doubles: sign(lambda_i)
     double2* d_coef = nullptr;     // k complex: c = V^+ x
     int cap_k = 0;
+    double2* d_coefb = nullptr;    // batched projector: k x 2 kBatch coefficient block
+    int cap_kb = 0;
 
     // deflation space of the multi-shift CG (borrowed W, eigenpairs of A = D_ov^+ D_ov; ov_set_deflation)
     const double2* Wdefl = nullptr;
@@ -189,6 +191,7 @@ int norm2_host(ov_ctx* ctx, const double2* x, double* out);
 struct MultiAxpyOuts {
     double2* out[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     double bscale[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    const double2* basej[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};  // overrides `base` for output j
 };
 int launch_multi_axpy(ov_ctx* ctx, const double2* xs, size_t stride, int nvec, int J, const double2* C_dev,
                       const double2* base, const MultiAxpyOuts& o);
@@ -200,8 +203,11 @@ int launch_combine_from_f32(ov_ctx* ctx, const float2* r, double a1, const doubl
 int ensure_gauge_f32(ov_ctx* ctx);
 int workspace_f32(ov_ctx* ctx, int i, float2** out);
 
+int launch_multi_dot_batch(ov_ctx* ctx, const double2* xs, size_t stride, int nvec, const double2* y, size_t ystride, int nb);
 // projector: c = V^+ x (left in ctx->d_result[0..k)); perp = x - V c; low = V (sgn o c)
 int project(ov_ctx* ctx, const double2* x, double2* perp, double2* low);
+// the same for nb consecutive right-hand sides (stride 12 V) with V streamed once per pass for groups of 4 / 2 of them
+int project_batch(ov_ctx* ctx, const double2* x, double2* perp, double2* low, int nb);
 
 // live timing: a Span records an event pair on ctx->stream around a phase when ctx->timing is on
 struct Span {

@@ -36,6 +36,53 @@ int project(ov_ctx* ctx, const double2* x, double2* perp, double2* low) {
     return launch_multi_axpy(ctx, ctx->Vlow, stride, ctx->k, 2, ctx->d_coef, x, o);
 }
 
+// C[i*2nb + 2r] = -c_{r,i} ; C[i*2nb + 2r+1] = sgn_i * c_{r,i}   (c_{r,i} = <v_i, x_r> at d_result[r*k + i])
+__global__ void projector_coef_batch_kernel(const double2* __restrict__ c, const double* __restrict__ sgn, int k, int nb,
+                                            double2* __restrict__ C) {
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= k * nb) return;
+    const int i = q % k, r = q / k;
+    const double2 v = c[q];
+    const double s = sgn[i];
+    C[(size_t)i * 2 * nb + 2 * r + 0] = make_double2(-v.x, -v.y);
+    C[(size_t)i * 2 * nb + 2 * r + 1] = make_double2(s * v.x, s * v.y);
+}
+
+// Batched projector: for a group of nb = 4 or 2 right-hand sides the eigenvectors
+// are streamed once for all V^+ x_r (multi_dot_kernel<nb>) and once for all 2 nb outputs (multi_axpy_kernel<2 nb>), so the
+// 2 k 192 B/site of the projector are paid per group, not per right-hand side.
+int project_batch(ov_ctx* ctx, const double2* x, double2* perp, double2* low, int nb) {
+    const size_t stride = spinor_elems(ctx);
+    int r0 = 0;
+    while (r0 < nb) {
+        const int g = (nb - r0 >= 4) ? 4 : (nb - r0 >= 2) ? 2 : 1;
+        if (g == 1) {
+            OV_TRY(project(ctx, x + r0 * stride, perp + r0 * stride, low + r0 * stride));
+        } else {
+            Span span(ctx, 1);
+            if (ctx->cap_kb < ctx->k * kBatch * 2) {
+                if (ctx->d_coefb) cudaFree(ctx->d_coefb);
+                ctx->d_coefb = nullptr;
+                ctx->cap_kb = 0;
+                OV_CUDA(ctx, cudaMalloc(&ctx->d_coefb, (size_t)ctx->k * kBatch * 2 * sizeof(double2)));
+                ctx->cap_kb = ctx->k * kBatch * 2;
+            }
+            OV_TRY(launch_multi_dot_batch(ctx, ctx->Vlow, stride, ctx->k, x + r0 * stride, stride, g));
+            projector_coef_batch_kernel<<<(ctx->k * g + 127) / 128, 128, 0, ctx->stream>>>(ctx->d_result, ctx->d_sgn, ctx->k, g, ctx->d_coefb);
+            ctx->launches++;
+            OV_CUDA(ctx, cudaGetLastError());
+            MultiAxpyOuts o;
+            for (int r = 0; r < g; r++) {
+                o.out[2 * r] = perp + (r0 + r) * stride; o.bscale[2 * r] = 1.0; o.basej[2 * r] = x + (r0 + r) * stride;
+                o.out[2 * r + 1] = low + (r0 + r) * stride; o.bscale[2 * r + 1] = 0.0;   // no base: starts from zero
+            }
+            OV_TRY(launch_multi_axpy(ctx, ctx->Vlow, stride, ctx->k, 2 * g, ctx->d_coefb, nullptr, o));
+        }
+        r0 += g;
+    }
+    return OV_OK;
+}
+
 // Wilson launch by precision
 static int wilson_t(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep, int nb) {
     return nb > 1 ? launch_wilson_batch(ctx, in, out, ep, nb) : launch_wilson(ctx, in, out, ep);
@@ -88,7 +135,7 @@ int sign_poly(ov_ctx* ctx, const double2* x, double2* out, const Epilogue& fin) 
     return clenshaw_t<double2>(ctx, ctx->coef.data(), n, x, out, fin, b1, b2, t);
 }
 
-// nb right-hand sides at once: per-rhs projector, then ONE Clenshaw sweep whose every launch covers the whole batch
+// nb right-hand sides at once: batched projector, then ONE Clenshaw sweep whose every launch covers the whole batch
 // (the links are then read from HBM once per site block and shared through L2/L1 by the right-hand sides).
 int apply_batch(ov_ctx* ctx, bool sign_only, double mass, const double2* in, double2* out, int nb) {
     if (ctx->order < 0) return fail(ctx, OV_ESTATE, "ov_set_polynomial has not been called");
@@ -98,7 +145,7 @@ int apply_batch(ov_ctx* ctx, bool sign_only, double mass, const double2* in, dou
     double2 *b1 = ctx->wsb, *b2 = b1 + kBatch * n, *t = b2 + kBatch * n, *perp = t + kBatch * n, *low = perp + kBatch * n;
     const double2* x = in;
     if (ctx->k > 0) {
-        for (int r = 0; r < nb; r++) OV_TRY(project(ctx, in + r * n, perp + r * n, low + r * n));
+        OV_TRY(project_batch(ctx, in, perp, low, nb));
         x = perp;
     }
     const int order = ctx->order;
