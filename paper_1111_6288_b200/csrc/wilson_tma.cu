@@ -97,11 +97,11 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
         "{\n"
         ".reg .pred p;\n"
         "WAIT_LOOP:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra WAIT_DONE;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n"   // %2: suspend-time hint, the warp sleeps in hardware
+        "@p bra WAIT_DONE;\n"                                             // instead of spinning on its scheduler's issue slots
         "bra WAIT_LOOP;\n"
         "WAIT_DONE:\n"
-        "}\n" ::"r"(bar), "r"(parity) : "memory");
+        "}\n" ::"r"(bar), "r"(parity), "r"(0x989680u) : "memory");
 }
 __device__ __forceinline__ void tma_load_5d(unsigned dst, const CUtensorMap* map, unsigned bar, int c0, int c1, int c2,
                                             int c3, int c4) {
@@ -282,9 +282,9 @@ __global__ void __launch_bounds__(Form<NA>::threads, 1) wilson_tma_kernel(const 
 #pragma unroll
             for (int k = 0; k < CH; k++) {
                 const long long e = gsite + (long long)(c0 + k) * a.V;
-                if (NA >= 1) w1[k] = a.A1[e];
-                if (NA >= 2) w2[k] = a.A2[e];
-                if (NA >= 3) w3[k] = a.A3[e];
+                if (NA >= 1) w1[k] = __ldcs(a.A1 + e);
+                if (NA >= 2) w2[k] = __ldcs(a.A2 + e);
+                if (NA >= 3) w3[k] = __ldcs(a.A3 + e);
             }
         };
         auto combine_store = [&](long long gsite, int c0, const double2* acc, const double2* w1, const double2* w2, const double2* w3) {
