@@ -8,9 +8,11 @@ Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl refere
   chebyshev.py       coefficients of P(x) ~ x^(-1/2) on [eps,1]; delta; eq. 2.2  (numpy)
   dense.py           dense H_w on tiny lattices, exact sign by eigendecomposition (numpy)
   multishift_cg.py   multi-shift CG on D_ov^dagger D_ov, step by step            (numpy)
+  deflation.py       D_ov^dagger D_ov per chirality sector, dense low modes, deflated multi-shift CG (numpy)
 
-Pins: tests/test_oracle_pins.py (see the table in DESIGN.md).  Unpinned: Lanczos completeness on
-lattices >= 16^3x32 ("parity unpinned" there: only residual/orthonormality are checked).
+Pins: tests/test_oracle_pins.py (see the table in DESIGN.md).  Parity unpinned: completeness of the D_ov low modes the
+CUDA library returns on lattices above 4^4 (residuals and the pairing of the chirality sectors are checked there, no
+independent eigensolver); H_w low modes are pinned at 8^4 by tests/golden/lowmodes_8x8x8x8.txt.
 """
 from .capi import (  # noqa: F401
     build,
