@@ -15,7 +15,7 @@ CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libov.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-         "-Xcompiler", "-fPIC", "-I", os.path.join(_ROOT, "include"), "-I", CSRC] + os.environ.get("OV_NVCC_FLAGS", "").split()
+         "-Xcompiler", "-fPIC", "-I", os.path.join(_ROOT, "include"), "-I", CSRC]
 
 
 def _sources():
