@@ -106,8 +106,10 @@ int ov_timing_read(ov_ctx* ctx, double* out_host);
 /* selects the Wilson kernel of single-right-hand-side launches: 0 = automatic (the TMA-staged kernel where it applies,
  * see DESIGN.md section 10), 1 = gather (one thread per site, operands through L1/L2; every shape and layout),
  * 2 = TMA-staged (persistent warp-specialised kernel: cp.async.bulk.tensor into shared-memory rings, mbarrier
- * producer/consumer; needs the planes layout and X % 8 == 0, Y % 4 == 0, Z % 4 == 0, else OV_EINVAL).  Both give
- * bit-identical results. */
+ * producer/consumer, an epilogue warpgroup for launches with fused axpy operands; needs the planes layout and
+ * X % 8 == 0, Y % 4 == 0, Z % 4 == 0, else OV_EINVAL).  The two kernels do the same arithmetic in the same order: the
+ * hopping term agrees to the last bit, results with an epilogue up to the compiler's FMA contraction (~2e-16 relative).
+ * Batched (nrhs > 1) and fp32 launches always use the gather kernel. */
 int ov_set_dslash_variant(ov_ctx* ctx, int variant);
 /* the variant single-right-hand-side Wilson launches of this context actually use (1 or 2; never 0) */
 int ov_get_dslash_variant(const ov_ctx* ctx);

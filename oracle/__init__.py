@@ -10,9 +10,9 @@ Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl refere
   multishift_cg.py   multi-shift CG on D_ov^dagger D_ov, step by step            (numpy)
   deflation.py       D_ov^dagger D_ov per chirality sector, dense low modes, deflated multi-shift CG (numpy)
 
-Pins: tests/test_oracle_pins.py (see the table in DESIGN.md).  Parity unpinned: completeness of the D_ov low modes the
-CUDA library returns on lattices above 4^4 (residuals and the pairing of the chirality sectors are checked there, no
-independent eigensolver); H_w low modes are pinned at 8^4 by tests/golden/lowmodes_8x8x8x8.txt.
+Pins: tests/test_oracle_pins.py (see the table in DESIGN.md).  Every function here has a pin.  What the GPU tests cannot
+check with it is completeness of the CUDA eigensolvers above 8^4 (H_w: tests/golden/lowmodes_8x8x8x8.txt; D_ov:
+tests/golden/dov_lowmodes_8x8x8x8.txt): on larger lattices eigenpairs are verified one by one, see DESIGN.md section 3.
 """
 from .capi import (  # noqa: F401
     build,

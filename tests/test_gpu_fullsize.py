@@ -379,3 +379,27 @@ def test_deflated_cg_16x32_hard_workload(ovp, parity_log):
     e = float(np.linalg.norm((b - Ax - sg * xh).ravel()) / np.linalg.norm(b.ravel()))
     parity_log("16^3x32 deflated solution, lightest mass: true residual with the ORACLE's D_ov", e, 2e-8)
     assert e <= 2e-8
+
+
+def test_dov_lowmodes_completeness_8x8_vs_oracle_eigsh(ovp, parity_log):
+    """No skipped D_ov mode (readings G20, G13): the k lowest mu per chirality sector
+    from ov_lanczos_dov_lowmodes with the production parameters (filter order 12, default subspace) equal the k lowest from
+    scipy's ARPACK run on the ORACLE's sector operator (tests/golden/dov_lowmodes_8x8x8x8.txt, written by
+    tests/golden/make_dov_lowmodes_golden.py) on an 8^4 lattice with smooth links and periodic time."""
+    from conftest import load_golden
+    g = load_golden("dov_lowmodes_8x8x8x8.txt")
+    dims, kappa, norm = (8, 8, 8, 8), 0.19, 1.0 + 8 * 0.19
+    se, n = float(g["sqrt_eps"]), int(g["order"])
+    U = wl.su3_links(dims, 0.3, wl.gauge_seed(8))
+    op = ovp.Overlap(dims, kappa, U, t_boundary="periodic")
+    op.set_polynomial(ovp.chebyshev_coeffs(n, se * se), se * se, norm)
+    for s, tag in ((+1, "p"), (-1, "m")):
+        gold = np.array([float(g[f"mu_{tag}_{i}"]) for i in range(10)])
+        for k in (8, 3):
+            W, mu, res, ok = op.lanczos_dov_lowmodes(s, k, tol=1e-10, max_restarts=60, cheb_order=12)
+            assert ok and np.all(res <= 1e-10)
+            err = float(np.max(np.abs(np.sort(mu) - gold[:k])))
+            parity_log(f"8^4 D_ov low modes, chirality {s:+d}, k={k} vs oracle+ARPACK: max |mu_i - golden_i| "
+                       f"({op.lanczos_stats()['restarts']} cycles)", err, 1e-9)
+            assert err <= 1e-9
+            assert mu.max() < gold[k] - 1e-9                             # nothing from above the k-th level
