@@ -421,7 +421,8 @@ def run_b200(args):
         yb = torch.empty_like(xb)
         ms_b = timed(lambda i: op.apply_dov(0.0, xb, yb), 1, 2)
         batched = {"nrhs": 4, "value": aggregate_value(world, 2 * 4, ms_b), "unit": UNIT,
-                   "note": "ov_apply_dov(nrhs=4): every Wilson launch covers 4 right-hand sides"}
+                   "note": "ov_apply_dov(nrhs=4): the small-space projector streams the eigenvectors once for the 4 right-hand sides; "
+                           "Clenshaw sweeps per right-hand side through the TMA-staged kernel (batched gather launches elsewhere)"}
         del xb, yb
 
     # ---- multi-mass CG time-to-solution on the same lattice (north_star: reported beside the headline)
