@@ -15,8 +15,8 @@
 //     no register spent on them and no __syncthreads between loading and computing;
 //   * consumers read neighbours and links from shared memory only (forward t neighbour = the next interior plane, which
 //     later becomes the site's own plane; the backward t hop U_t(x-t)^+ (1+gamma_t) psi(x-t) is carried in registers
-//     from the previous step), do the same arithmetic in the same order as the gather kernel (results are bit-identical),
-//     and store the result with coalesced 16-byte stores.
+//     from the previous step), do the same arithmetic in the same order as the gather kernel (the hop is bit-identical,
+//     results with an epilogue agree up to the compiler's FMA contraction) and store with coalesced 16-byte stores;
 //   * launches with fused axpy operands (NA >= 1: the second launch of every Clenshaw order, the D_ov assembly) add an
 //     EPILOGUE warpgroup: the consumers hand their accumulators over through a 24 KB shared-memory buffer and go on with
 //     the next slice, while four epilogue warps -- which hold nothing else in registers -- issue the operand loads of a
