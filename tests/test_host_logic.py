@@ -83,3 +83,17 @@ def test_bench_algorithmic_bytes():
     assert per_site == n * 2496 - 192 + 960 + 384          # 2496 B/site per order
     assert bench.algorithmic_bytes_per_sign(n, 1, True, recon=12) == per_site - (2 * n + 1) * 192
     assert bench.aggregate_value(1, 8, 1000.0) == 8.0
+
+
+def test_options_struct_matches_header():
+    """binding.OvOptions mirrors struct ov_options of include/ov.h field by field (6 ints + 1 double = 32 bytes)."""
+    import ctypes
+    import re
+    from paper_1111_6288_b200.binding import OvOptions
+    src = open(os.path.join(ROOT, "include", "ov.h")).read()
+    body = re.search(r"typedef struct ov_options \{(.*?)\} ov_options;", src, re.S).group(1)
+    body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
+    fields = [(m.group(1), m.group(2)) for m in re.finditer(r"(int|double)\s+(\w+)\s*;", body)]
+    ctype = {"int": ctypes.c_int, "double": ctypes.c_double}
+    assert [(n, ctype[t]) for t, n in fields] == list(OvOptions._fields_)
+    assert ctypes.sizeof(OvOptions) == 32
