@@ -191,7 +191,9 @@ static int launch_gather_t(ov_ctx* ctx, const C* gauge, const C* in, C* out, con
     a.reverse = ctx->flip;
     ctx->flip ^= 1;
     const int threads = GatherShape<C>::threads;
-    const unsigned blocks = (unsigned)((a.V + threads - 1) / threads) * (unsigned)a.nrb;
+    const long long nblocks = ((a.V + threads - 1) / threads) * (long long)a.nrb;
+    if (nblocks > 0x7fffffffLL) return fail(ctx, OV_EINVAL, "too many right-hand sides for one launch (%lld blocks)", nblocks);
+    const unsigned blocks = (unsigned)nblocks;
     const dim3 bdim(threads, rb);
     const int na = ep.hop_only ? -1 : (ep.A3 ? 3 : ep.A2 ? 2 : ep.A1 ? 1 : 0);
     if ((ep.A3 && !ep.A2) || (ep.A2 && !ep.A1)) return fail(ctx, OV_EINVAL, "epilogue operands must be filled in order");
