@@ -541,3 +541,38 @@ def test_degenerate_inputs(ovp, cfg0):
         op.apply_dov_reduced(0.0, zero, cfg.order + 1, False)
     with pytest.raises(ovp.OvError):
         ovp.Overlap((4, 4, 4, 1), KAPPA, wl.unit_links((4, 4, 4, 1)))   # every extent must be >= 2
+
+
+def test_deflation_degenerate_inputs(ovp):
+    """Edge cases of the deflation row: bad arguments are refused; a source that lies inside the deflation space is solved
+    with zero CG iterations, x_i = w (w^+ b)/(mu + sigma_i); clearing the deflation space restores the plain solver."""
+    dims = (4, 4, 4, 4)
+    U = wl.su3_links(dims, 0.3, 41)
+    with oracle.boundary((1.0, 1.0, 1.0, 1.0)):
+        w, _, _, _ = dense.eig_hw(dims, KAPPA, U)
+    se = 0.9 * np.min(np.abs(w)) / NORM
+    # the defect 1 - sign^2 = O(delta) of a sector eigenvector enters x amplified by 1/(mu + sigma) ~ 1e3 here
+    # (include/ov.h, ov_set_deflation): delta ~ 1e-13 by eq. 2.2
+    n = int(np.ceil(np.log(0.41 / 1e-13) / (2.1 * se)))
+    op = ovp.Overlap(dims, KAPPA, U, t_boundary="periodic")
+    with pytest.raises(ovp.OvError):
+        op.lanczos_dov_lowmodes(+1, 2)                        # no polynomial yet
+    op.set_polynomial(ovp.chebyshev_coeffs(n, se * se), se * se, NORM)
+    for bad in (dict(chirality=0, k=2), dict(chirality=2, k=2), dict(chirality=1, k=0)):
+        with pytest.raises(ovp.OvError):
+            op.lanczos_dov_lowmodes(bad["chirality"], bad["k"])
+    W, mu, res, ok = op.lanczos_dov_lowmodes(-1, 3, tol=1e-12, max_restarts=80, cheb_order=12, subspace=30)
+    assert ok
+    with pytest.raises(ovp.OvError):
+        op.set_deflation(W, -np.abs(mu) - 1.0)                # D^+ D has no negative eigenvalue
+    op.set_deflation(W, mu)
+    masses = (0.01, 0.1)
+    b = W[1].clone()                                          # a source inside the deflation space
+    x, iters, relres, okc = op.multishift_cg(masses, b, tol=1e-8, maxiter=100)
+    assert okc and iters == 0 and np.all(relres <= 1e-8)
+    bh, xh = to_host(op, b), to_host(op, x)
+    for i, m in enumerate(masses):
+        assert rel(xh[i], bh / (mu[1] + sigma_of_mass(m))) <= 1e-8
+    op.set_deflation(None, None)
+    _, iters2, relres2, ok2 = op.multishift_cg(masses, b, tol=1e-8, maxiter=500)
+    assert ok2 and iters2 > 0 and np.all(relres2 <= 1e-8)
