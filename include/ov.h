@@ -163,6 +163,11 @@ int ov_apply_dov_reduced(ov_ctx* ctx, double mass, const void* in, void* out, in
 /* test/bench hook: out = H_w in computed by the SINGLE-precision instantiation of the Wilson kernel (in is rounded to
  * fp32, the links are the fp32 copy the adaptive CG uses, the result is widened to fp64).  One right-hand side.       */
 int ov_apply_hw_f32(ov_ctx* ctx, const void* in, void* out);
+/* host-buffer entry points (what bench.py's e2e times): in_host / out_host are nrhs CANONICAL spinors in HOST memory; each
+ * right-hand side is copied to the device, re-laid out, run through the operator, re-laid out and copied back.  With
+ * nrhs > 1 the copies run on two internal copy streams (double-buffered staging), so the H2D of right-hand side r+1 and
+ * the D2H of r-1 overlap the operator on r; pinned host memory is needed for that overlap (pageable memory works, copies
+ * then serialise).  The call returns when out_host is complete.                                                       */
 int ov_apply_hw_host(ov_ctx* ctx, const void* in_host, void* out_host, int nrhs);
 int ov_apply_dov_host(ov_ctx* ctx, double mass, const void* in_host, void* out_host, int nrhs);
 

@@ -232,13 +232,15 @@ class Overlap:
         n = self.lib.ov_cg_orders(self._ctx, buf, ctypes.c_int(4096))
         return [buf[i] for i in range(min(n, 4096))]
 
-    def apply_hw_host(self, x_host: np.ndarray) -> np.ndarray:
-        """canonical HOST array in, canonical HOST array out (H2D and D2H inside the call)."""
-        x = np.ascontiguousarray(x_host, dtype=np.complex128)
-        out = np.empty_like(x)
-        nrhs = x.size // (12 * self.V)
-        self._check(self.lib.ov_apply_hw_host(self._ctx, _ptr(x), _ptr(out), ctypes.c_int(nrhs)))
-        return out
+    def apply_hw_host(self, x_host, out_host=None):
+        """canonical HOST array (numpy or torch, pinned for asynchronous copies) in, canonical HOST array out (H2D and
+        D2H inside the call)."""
+        x = x_host if isinstance(x_host, torch.Tensor) else np.ascontiguousarray(x_host, dtype=np.complex128)
+        if out_host is None:
+            out_host = torch.empty_like(x) if isinstance(x, torch.Tensor) else np.empty_like(x)
+        nrhs = (x.numel() if isinstance(x, torch.Tensor) else x.size) // (12 * self.V)
+        self._check(self.lib.ov_apply_hw_host(self._ctx, _ptr(x), _ptr(out_host), ctypes.c_int(nrhs)))
+        return out_host
 
     def apply_dov_host(self, mass, x_host, out_host=None):
         x = x_host if isinstance(x_host, torch.Tensor) else np.ascontiguousarray(x_host, dtype=np.complex128)

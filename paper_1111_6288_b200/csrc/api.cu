@@ -180,9 +180,20 @@ void ov_destroy(ov_ctx* ctx) {
     cudaFree(ctx->d_sgn);
     cudaFree(ctx->d_coef);
     cudaFree(ctx->d_coefb);
-    cudaFree(ctx->host_stage_in);
-    cudaFree(ctx->host_stage_abi);
-    cudaFree(ctx->host_stage_out);
+    {
+        HostPipe& hp = ctx->host_pipe;
+        if (hp.h2d) { cudaStreamSynchronize(hp.h2d); cudaStreamDestroy(hp.h2d); }
+        if (hp.d2h) { cudaStreamSynchronize(hp.d2h); cudaStreamDestroy(hp.d2h); }
+        for (int b = 0; b < 2; b++) {
+            cudaFree(hp.cin[b]); cudaFree(hp.cout[b]);
+            if (hp.in_ready[b]) cudaEventDestroy(hp.in_ready[b]);
+            if (hp.in_free[b]) cudaEventDestroy(hp.in_free[b]);
+            if (hp.out_ready[b]) cudaEventDestroy(hp.out_ready[b]);
+            if (hp.out_free[b]) cudaEventDestroy(hp.out_free[b]);
+        }
+        cudaFree(hp.abi_in); cudaFree(hp.abi_out);
+        if (hp.start) cudaEventDestroy(hp.start);
+    }
     for (auto e : ctx->ev_pool) cudaEventDestroy(e);
     tma_state_free(ctx);
     delete ctx;

@@ -156,26 +156,56 @@ int ov_cg_orders(const ov_ctx* ctx, int* out_host, int cap) {
     return n;
 }
 
-// host-buffer path: H2D -> pack -> operator -> unpack -> D2H, one RHS at a time through 3 device stages
+// host-buffer path: H2D -> pack -> operator -> unpack -> D2H.  With nrhs > 1 the copies run on two copy streams (one per
+// direction, double-buffered canonical staging): the H2D of right-hand side r+1 and the D2H of r-1 overlap the operator on r,
+// so only the first H2D and the last D2H are exposed.  Host buffers should be pinned for the copies to be asynchronous.
 static int host_apply(ov_ctx* ctx, int which, double mass, const void* in_host, void* out_host, int nrhs) {
     if (!ctx) return OV_EINVAL;
     if (!in_host || !out_host || nrhs < 1) return fail(ctx, OV_EINVAL, "null pointer or nrhs < 1");
     const size_t n = spinor_elems(ctx), bytes = n * sizeof(double2);
-    if (!ctx->host_stage_in) OV_CUDA(ctx, cudaMalloc(&ctx->host_stage_in, bytes));
-    if (!ctx->host_stage_abi) OV_CUDA(ctx, cudaMalloc(&ctx->host_stage_abi, bytes));
-    if (!ctx->host_stage_out) OV_CUDA(ctx, cudaMalloc(&ctx->host_stage_out, bytes));
+    HostPipe& hp = ctx->host_pipe;
+    if (!hp.ready) {
+        for (int b = 0; b < 2; b++) {
+            OV_CUDA(ctx, cudaMalloc(&hp.cin[b], bytes));
+            OV_CUDA(ctx, cudaMalloc(&hp.cout[b], bytes));
+            OV_CUDA(ctx, cudaEventCreateWithFlags(&hp.in_ready[b], cudaEventDisableTiming));
+            OV_CUDA(ctx, cudaEventCreateWithFlags(&hp.in_free[b], cudaEventDisableTiming));
+            OV_CUDA(ctx, cudaEventCreateWithFlags(&hp.out_ready[b], cudaEventDisableTiming));
+            OV_CUDA(ctx, cudaEventCreateWithFlags(&hp.out_free[b], cudaEventDisableTiming));
+        }
+        OV_CUDA(ctx, cudaMalloc(&hp.abi_in, bytes));
+        OV_CUDA(ctx, cudaMalloc(&hp.abi_out, bytes));
+        OV_CUDA(ctx, cudaStreamCreateWithFlags(&hp.h2d, cudaStreamNonBlocking));
+        OV_CUDA(ctx, cudaStreamCreateWithFlags(&hp.d2h, cudaStreamNonBlocking));
+        OV_CUDA(ctx, cudaEventCreateWithFlags(&hp.start, cudaEventDisableTiming));
+        hp.ready = true;
+    }
+    // the copy streams start after everything the caller enqueued on the context's stream so far
+    OV_CUDA(ctx, cudaEventRecord(hp.start, ctx->stream));
+    OV_CUDA(ctx, cudaStreamWaitEvent(hp.h2d, hp.start, 0));
+    OV_CUDA(ctx, cudaStreamWaitEvent(hp.d2h, hp.start, 0));
     for (int r = 0; r < nrhs; r++) {
-        OV_CUDA(ctx, cudaMemcpyAsync(ctx->host_stage_in, (const char*)in_host + r * bytes, bytes, cudaMemcpyHostToDevice, ctx->stream));
-        OV_TRY(launch_pack(ctx, ctx->host_stage_in, ctx->host_stage_abi));
+        const int b = r & 1;
+        if (r >= 2) OV_CUDA(ctx, cudaStreamWaitEvent(hp.h2d, hp.in_free[b], 0));       // pack of r-2 has consumed cin[b]
+        OV_CUDA(ctx, cudaMemcpyAsync(hp.cin[b], (const char*)in_host + r * bytes, bytes, cudaMemcpyHostToDevice, hp.h2d));
+        OV_CUDA(ctx, cudaEventRecord(hp.in_ready[b], hp.h2d));
+        OV_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, hp.in_ready[b], 0));
+        OV_TRY(launch_pack(ctx, hp.cin[b], hp.abi_in));
+        OV_CUDA(ctx, cudaEventRecord(hp.in_free[b], ctx->stream));
         if (which == 0) {
             Epilogue ep;
-            OV_TRY(launch_wilson(ctx, ctx->host_stage_abi, ctx->host_stage_out, ep));
+            OV_TRY(launch_wilson(ctx, hp.abi_in, hp.abi_out, ep));
         } else {
-            OV_TRY(apply_dov(ctx, mass, ctx->host_stage_abi, ctx->host_stage_out));
+            OV_TRY(apply_dov(ctx, mass, hp.abi_in, hp.abi_out));
         }
-        OV_TRY(launch_unpack(ctx, ctx->host_stage_out, ctx->host_stage_in));
-        OV_CUDA(ctx, cudaMemcpyAsync((char*)out_host + r * bytes, ctx->host_stage_in, bytes, cudaMemcpyDeviceToHost, ctx->stream));
+        if (r >= 2) OV_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, hp.out_free[b], 0)); // D2H of r-2 has drained cout[b]
+        OV_TRY(launch_unpack(ctx, hp.abi_out, hp.cout[b]));
+        OV_CUDA(ctx, cudaEventRecord(hp.out_ready[b], ctx->stream));
+        OV_CUDA(ctx, cudaStreamWaitEvent(hp.d2h, hp.out_ready[b], 0));
+        OV_CUDA(ctx, cudaMemcpyAsync((char*)out_host + r * bytes, hp.cout[b], bytes, cudaMemcpyDeviceToHost, hp.d2h));
+        OV_CUDA(ctx, cudaEventRecord(hp.out_free[b], hp.d2h));
     }
+    OV_CUDA(ctx, cudaStreamSynchronize(hp.d2h));
     OV_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     return OV_OK;
 }

@@ -59,6 +59,18 @@ using EpilogueF = EpilogueT<float2>;
 
 }  // namespace ov
 
+// staging of the *_host entry points (api_ops.cu::host_apply)
+struct HostPipe {
+    bool ready = false;
+    double2* cin[2] = {nullptr, nullptr};    // canonical input, double-buffered
+    double2* cout[2] = {nullptr, nullptr};   // canonical output, double-buffered
+    double2* abi_in = nullptr;
+    double2* abi_out = nullptr;
+    cudaStream_t h2d = nullptr, d2h = nullptr;
+    cudaEvent_t start = nullptr, in_ready[2] = {nullptr, nullptr}, in_free[2] = {nullptr, nullptr},
+                out_ready[2] = {nullptr, nullptr}, out_free[2] = {nullptr, nullptr};
+};
+
 struct ov_ctx {
     ov::Lattice lat{};
     double kappa = 0.0;
@@ -105,9 +117,7 @@ struct ov_ctx {
     double2* d_result = nullptr;   // reduced results (device)
     size_t result_cap = 0;
     double2* h_result = nullptr;   // pinned host mirror
-    double2* host_stage_in = nullptr;   // device staging for *_host calls (canonical)
-    double2* host_stage_abi = nullptr;
-    double2* host_stage_out = nullptr;
+    HostPipe host_pipe;
 
     // live timing (ov_timing_enable): CUDA-event pairs on ctx->stream around the two phases of an apply
     bool timing = false;

@@ -125,11 +125,21 @@ def test_hw_rejects_aliasing_and_bad_args(ovp):
 def test_hw_host_entry_point(ovp):
     dims = (4, 2, 6, 8)
     U = wl.su3_links(dims, 0.5, 5)
-    x = np.stack([wl.gaussian_source(dims, 6), wl.gaussian_source(dims, 7)])
+    x = np.stack([wl.gaussian_source(dims, 6 + j) for j in range(5)])   # 5 rhs: both staging buffers are re-used twice
     op = make(ovp, dims, U)
-    got = op.apply_hw_host(x)
     ref = np.stack([oracle.hw(dims, KAPPA, U, v) for v in x])
+    got = op.apply_hw_host(x)                                            # pageable host memory
     assert rel(got, ref) <= TOL_HW
+    xp = torch.from_numpy(x).pin_memory()                                # pinned: H2D / D2H overlap the operator
+    outp = torch.empty_like(xp).pin_memory()
+    for _ in range(2):                                                   # a second call re-uses the pipeline
+        outp.zero_()
+        op.apply_hw_host(xp, outp)
+        assert rel(outp.numpy(), ref) <= TOL_HW
+    op.set_polynomial(ovp.chebyshev_coeffs(6, 0.04), 0.04, NORM)
+    gd = op.apply_dov_host(0.1, xp[:3].contiguous().pin_memory())
+    for j in range(3):
+        assert rel(gd[j].numpy(), oracle.dov(dims, KAPPA, U, ovp.chebyshev_coeffs(6, 0.04), 0.04, NORM, None, None, 0.1, x[j])) <= TOL_DOV
 
 
 # ------------------------------------------------------------------------------------------ BLAS-1
