@@ -76,8 +76,9 @@ int ov_create(ov_ctx** out, const int dims[4], double kappa, const void* gauge_d
  *               "U_mu -> exp(-i q A_mu) U_mu"), in the gauge A_t(x) = E (x_dir - field_origin), other components zero
  *               (reading G19: the paper does not fix the gauge): the library's copy of every t link is
  *               multiplied by exp(-i field_qE (x_dir - field_origin)), field_qE = q E in lattice units.  The links
- *               are then U(3), so field != 0 needs recon = 18 (OV_EINVAL otherwise); with recon = 12 the SU(3) check
- *               applies to the caller's links, walls are allowed.                                                  */
+ *               are then U(3).  recon = 18 stores them whole; recon = 12 keeps rows 0-1 (with the phase) and the kernels
+ *               multiply the rebuilt third row by det U = exp(-3 i field_qE (x_dir - field_origin)) (phase-tracked
+ *               reconstruction), so the caller's links must be SU(3) as always with recon = 12.                       */
 enum { OV_BC_ANTIPERIODIC = 0, OV_BC_PERIODIC = 1, OV_BC_OPEN = 2 };
 typedef struct ov_options {
     int layout;

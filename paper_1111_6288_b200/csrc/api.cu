@@ -126,7 +126,7 @@ int ov_create_ex(ov_ctx** out, const int dims[4], double kappa, const void* gaug
     if (options) opt = *options;
     if (opt.layout < 0 || opt.layout > 2 || opt.t_boundary < 0 || opt.t_boundary > 2) return OV_EINVAL;
     if (opt.reserved != 0 || opt.wall_mask < 0 || opt.wall_mask > 7 || opt.field < 0 || opt.field > 3) return OV_EINVAL;
-    if (opt.field != 0 && (recon != 18 || !std::isfinite(opt.field_qE))) return OV_EINVAL;   // U(3) links need all 18 reals
+    if (opt.field != 0 && !std::isfinite(opt.field_qE)) return OV_EINVAL;
     *out = nullptr;
     if (!dims || !gauge_dev) return OV_EINVAL;
     if (recon != 18 && recon != 12) return OV_EINVAL;
@@ -143,6 +143,9 @@ int ov_create_ex(ov_ctx** out, const int dims[4], double kappa, const void* gaug
     if (opt.layout == 1 && ctx->lat.V % 32 != 0) { delete ctx; return OV_EINVAL; }
     ctx->blocked = opt.layout == 1 || (opt.layout == 0 && ctx->lat.V % 32 == 0 && !tma_eligible(ctx->lat));
     ctx->t_phase = opt.t_boundary == OV_BC_PERIODIC ? 1.0 : opt.t_boundary == OV_BC_OPEN ? 0.0 : -1.0;
+    ctx->field_dir = opt.field - 1;
+    ctx->field_qE = opt.field_qE;
+    ctx->field_origin = opt.field_origin;
     ctx->stream = (cudaStream_t)cuda_stream;
     const size_t gbytes = gauge_elems(ctx->lat.V, recon) * sizeof(double2);
     cudaError_t e = cudaMalloc(&ctx->gauge, gbytes);

@@ -80,6 +80,9 @@ struct ov_ctx {
     float2* gauge_f = nullptr; // fp32 copy of the links, same layout (made on first use by the adaptive CG)
     int dslash_variant = 0;    // ov_set_dslash_variant: 0 automatic, 1 gather, 2 TMA-staged
     double t_phase = -1.0;     // factor on the hop across the t boundary (ov_options::t_boundary)
+    int field_dir = -1;        // background field (ov_options::field - 1), its strength q E and origin: the links already carry
+    double field_qE = 0.0;     // it; the Wilson kernels need it only to rebuild the third row of 12-real t links
+    int field_origin = 0;
     void* tma_state = nullptr; // tensor maps and schedule of the TMA-staged kernel (wilson_tma.cu)
     std::vector<int> cg_orders;  // order used at each iteration of the last adaptive CG (negative: fp32 sweep)
     std::array<double, 6> lanczos_stats{};  // last ov_lanczos_lowmodes: restarts, filter applies, launches, edge a, widenings, m

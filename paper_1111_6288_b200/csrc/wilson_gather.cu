@@ -24,6 +24,9 @@ struct GatherArgs {
     long long V;
     double kappa;
     double tphase;         // factor on the hop across the t boundary: -1 antiperiodic, +1 periodic, 0 open
+    int field_dir;         // background field (ov_options.field - 1; -1 = none): with 12-real links the rebuilt third row of a
+    double field_3qE;      // t link is multiplied by exp(-3 i qE (x_dir - origin)) = det of the U(3) link (phase-tracked recon)
+    int field_origin;
     int reverse;
     int nrb;               // rhs groups per site block (batched launch): block id = site_block * nrb + rhs_group
     long long rhs_stride;  // elements between consecutive right-hand sides in in/out/A1..A3
@@ -47,10 +50,17 @@ __device__ __forceinline__ void load_link(const C* __restrict__ gauge, long long
     for (int e = 0; e < NE; e++) u[e] = __ldg(p + (long long)e * es);
     if (RECON == 12) su3_row2(u);
 }
+// 12-real links that carry a U(1) phase (background field): rows 0-1 are stored with the phase, so conj(row0 x row1) is
+// the true third row times conj(det U) -- multiply it by det U = w
+template <typename C>
+__device__ __forceinline__ void row2_phase(C* __restrict__ u, C w) {
+#pragma unroll
+    for (int e = 6; e < 9; e++) u[e] = cmul(u[e], w);
+}
 
 template <int MU, int SIGMA, int RECON, bool BL, typename C>
 __device__ __forceinline__ void hop(C* __restrict__ acc, const GatherArgs<C>& a, long long nsite, long long lsite,
-                                    real_t<C> ph) {
+                                    real_t<C> ph, const C* det = nullptr) {
     C psi[12], h[6], g[6], u[9];
     const C* pn = a.in + spinor_base<BL>(nsite);
     const long long cs = spinor_stride<BL>(a.V);
@@ -58,6 +68,7 @@ __device__ __forceinline__ void hop(C* __restrict__ acc, const GatherArgs<C>& a,
     for (int c = 0; c < 12; c++) psi[c] = __ldg(pn + c * cs);
     project<MU, SIGMA>(psi, h);
     load_link<RECON, BL>(a.gauge, a.V, MU, lsite, u);
+    if (RECON == 12 && MU == 3 && det) row2_phase(u, *det);
     su3_mul<(SIGMA > 0)>(u, h, g);
     reconstruct_add<MU, SIGMA>(acc, g, ph);
 }
@@ -124,8 +135,16 @@ wilson_gather_kernel(GatherArgs<C> a) {
         const bool wp = (t + 1 == a.T), wm = (t == 0);
         const long long ip = wp ? i - (a.T - 1) * sT : i + sT;
         const long long im = wm ? i + (a.T - 1) * sT : i - sT;
-        hop<3, -1, RECON, BL>(acc, a, ip, i, wp ? (R)a.tphase : (R)1);  // boundary in time (default antiperiodic)
-        hop<3, +1, RECON, BL>(acc, a, im, im, wm ? (R)a.tphase : (R)1);
+        C det = cmake<C>(1, 0);   // det of this site's t links (they depend on the space coordinates only)
+        const bool field = RECON == 12 && a.field_dir >= 0;
+        if (field) {
+            const int xd = a.field_dir == 0 ? x : a.field_dir == 1 ? y : z;
+            double sn, cs;
+            sincos(-a.field_3qE * (double)(xd - a.field_origin), &sn, &cs);
+            det = cmake<C>((R)cs, (R)sn);
+        }
+        hop<3, -1, RECON, BL>(acc, a, ip, i, wp ? (R)a.tphase : (R)1, field ? &det : nullptr);  // boundary in time
+        hop<3, +1, RECON, BL>(acc, a, im, im, wm ? (R)a.tphase : (R)1, field ? &det : nullptr);
     }
 
     const EpilogueT<C>& ep = a.ep;
@@ -187,6 +206,9 @@ static int launch_gather_t(ov_ctx* ctx, const C* gauge, const C* in, C* out, con
     a.V = ctx->lat.V;
     a.kappa = ctx->kappa;
     a.tphase = ctx->t_phase;
+    a.field_dir = ctx->field_dir;
+    a.field_3qE = 3.0 * ctx->field_qE;
+    a.field_origin = ctx->field_origin;
     a.ep = ep;
     a.reverse = ctx->flip;
     ctx->flip ^= 1;

@@ -80,6 +80,9 @@ struct Args {
     int nitems;
     int reverse;
     double tphase;          // factor on the hop across the t boundary: -1 antiperiodic, +1 periodic, 0 open
+    int field_dir;          // background field (-1 = none): with 12-real links the rebuilt third row of a t link is multiplied
+    double field_3qE;       // by det U = exp(-3 i qE (x_dir - origin))  (phase-tracked reconstruction)
+    int field_origin;
 };
 
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -144,11 +147,16 @@ __device__ __forceinline__ void lds_link(const double2* p, int stride, double2* 
 }
 
 template <int MU, int SIGMA, int RECON>
-__device__ __forceinline__ void hop_smem(double2* acc, const double2* pn, int ns, const double2* pl, int ls, double ph) {
+__device__ __forceinline__ void hop_smem(double2* acc, const double2* pn, int ns, const double2* pl, int ls, double ph,
+                                         const double2* det = nullptr) {
     double2 psi[12], h[6], g[6], u[9];
     lds_spinor(pn, ns, psi);
     project<MU, SIGMA>(psi, h);
     lds_link<RECON>(pl, ls, u);
+    if (RECON == 12 && det) {
+#pragma unroll
+        for (int e = 6; e < 9; e++) u[e] = cmul(u[e], *det);
+    }
     su3_mul<(SIGMA > 0)>(u, h, g);
     reconstruct_add<MU, SIGMA>(acc, g, ph);
 }
@@ -339,6 +347,19 @@ __global__ void __launch_bounds__(Form<NA>::threads, 1) wilson_tma_kernel(const 
     for (int it = blockIdx.x; it < a.nitems; it += gridDim.x) {
         const Item w = decode_item(a, it);
         double2 P[6];   // U_t(x, t-1)^+ (1 + gamma_t) psi(x, t-1): the backward-t hop of the next step, before the boundary sign
+        // 12-real links in a background field: det of this site's t links (it depends on the space coordinates only)
+        const bool field = RECON == 12 && a.field_dir >= 0;
+        double2 det = make_double2(1.0, 0.0);
+        if (field) {
+            const int xd = a.field_dir == 0 ? w.x0 + lx : a.field_dir == 1 ? w.y0 + ly : w.z0 + lz;
+            sincos(-a.field_3qE * (double)(xd - a.field_origin), &det.y, &det.x);
+        }
+        auto fix_row2 = [&](double2* u) {
+            if (field) {
+#pragma unroll
+                for (int e = 6; e < 9; e++) u[e] = cmul(u[e], det);
+            }
+        };
         {   // ---- prologue: slice t0 - 1
             const unsigned si = slot_of<SI>(nI), sl = slot_of<SL>(nL);
             mbar_wait(fullI(si), full_parity<SI>(nI));
@@ -349,6 +370,7 @@ __global__ void __launch_bounds__(Form<NA>::threads, 1) wilson_tma_kernel(const 
             lds_spinor(Ib, SITES, psi);
             project<3, +1>(psi, h);
             lds_link<RECON>(Lb, SITES, u);
+            fix_row2(u);
             su3_mul<true>(u, h, P);
             release(emptyI(si));
             release(emptyL(sl));
@@ -420,13 +442,14 @@ __global__ void __launch_bounds__(Form<NA>::threads, 1) wilson_tma_kernel(const 
                 mbar_wait(fullI(s1), full_parity<SI>(nI + 1));
                 const double2* Lb = (const double2*)(sL + sl * L_BYTES) + sin;
                 const double2* I1 = (const double2*)(sI + s1 * I_BYTES) + sin;
-                hop_smem<3, -1, RECON>(acc, I1, SITES, Lb, SITES, (t + 1 == a.T) ? a.tphase : 1.0);   // boundary in time
+                hop_smem<3, -1, RECON>(acc, I1, SITES, Lb, SITES, (t + 1 == a.T) ? a.tphase : 1.0, field ? &det : nullptr);   // boundary in time
                 reconstruct_add<3, +1>(acc, P, (t == 0) ? a.tphase : 1.0);
                 // the product the next slice needs: U_t(x,t)^+ (1 + gamma_t) psi(x,t)
                 double2 psi[12], h[6], u[9];
                 lds_spinor(I0, SITES, psi);
                 project<3, +1>(psi, h);
                 lds_link<RECON>(Lb, SITES, u);
+                fix_row2(u);
                 su3_mul<true>(u, h, P);
                 release(emptyL(sl));
                 nL++;
@@ -606,6 +629,9 @@ int launch_wilson_tma(ov_ctx* ctx, const double2* in, double2* out, const Epilog
     a.reverse = ctx->flip;
     ctx->flip ^= 1;
     a.tphase = ctx->t_phase;
+    a.field_dir = ctx->field_dir;
+    a.field_3qE = 3.0 * ctx->field_qE;
+    a.field_origin = ctx->field_origin;
     if ((ep.A3 && !ep.A2) || (ep.A2 && !ep.A1)) return fail(ctx, OV_EINVAL, "epilogue operands must be filled in order");
     const int na = ep.hop_only ? -1 : (ep.A3 ? 3 : ep.A2 ? 2 : ep.A1 ? 1 : 0);
     const int grid = st->nitems < st->sm_count ? st->nitems : st->sm_count;

@@ -449,12 +449,16 @@ def test_background_field_and_boundaries_api_vs_oracle(ovp, variant, t_boundary,
     assert rel(to_host(op, op.apply_hw(dx)), ref_h) <= TOL_HW
     assert rel(to_host(op, op.apply_dov(0.05, dx)), ref_d) <= TOL_DOV
     assert rel(ref_h, oracle.hw(dims, KAPPA, U, x)) > 1e-3               # the field and the walls do matter
-    with pytest.raises(ovp.OvError):                                     # U(3) links cannot be rebuilt from 12 reals
-        ovp.Overlap(dims, KAPPA, U, recon=12, field_dir=fdir, field_qE=qE)
-    op12 = ovp.Overlap(dims, KAPPA, U, recon=12, t_boundary=t_boundary, walls=(fdir,))   # walls alone: fine with recon 12
-    with oracle.boundary(bc):
-        ref12 = oracle.hw(dims, KAPPA, U, x)
-    assert rel(to_host(op12, op12.apply_hw(to_dev(op12, x))), ref12) <= TOL_HW
+    # 12-real links: rows 0-1 carry the field's phase, the kernels multiply the rebuilt third row by det U (phase-tracked
+    # reconstruction) -- same operator, both Wilson kernels, and the fp32 instantiation of the gather kernel
+    op12 = ovp.Overlap(dims, KAPPA, U, recon=12, t_boundary=t_boundary, walls=(fdir,), field_dir=fdir, field_qE=qE,
+                       field_origin=org)
+    op12.set_dslash_variant(variant)
+    op12.set_polynomial(coef, se * se, NORM)
+    d12 = to_dev(op12, x)
+    assert rel(to_host(op12, op12.apply_hw(d12)), ref_h) <= TOL_HW
+    assert rel(to_host(op12, op12.apply_dov(0.05, d12)), ref_d) <= TOL_DOV
+    assert rel(to_host(op12, op12.apply_hw_f32(d12)), ref_h) <= 5e-7
 
 
 # ------------------------------------------------------------------------------------------ D_ov low modes, deflated CG
