@@ -75,7 +75,8 @@ def test_pack_unpack_roundtrip(ovp):
 @pytest.mark.parametrize("dims,spread", [((4, 4, 4, 4), 0.3), ((4, 2, 6, 8), 0.6), ((8, 8, 8, 16), 0.5),
                                          ((24, 4, 4, 2), 0.8), ((6, 10, 2, 4), 0.4), ((6, 6, 2, 6), 0.5),
                                          ((2, 2, 2, 2), 0.7), ((8, 4, 4, 3), 0.6), ((16, 8, 4, 6), 0.7),
-                                         ((8, 12, 8, 5), 0.5)])
+                                         ((8, 12, 8, 5), 0.5), ((8, 4, 4, 2), 0.6), ((24, 8, 12, 4), 0.7),
+                                         ((32, 4, 8, 3), 0.5)])
 @pytest.mark.parametrize("recon", [18, 12])
 def test_dslash_and_hw_vs_oracle(ovp, dims, spread, recon):
     U = wl.su3_links(dims, spread, wl.gauge_seed(1))
