@@ -22,6 +22,10 @@ The paper gives no formula, so the plain definitions are written out (DESIGN.md 
     eigenvectors of the SAME A the CG applies, to the CG tolerance: with a polynomial sign of error delta the sector
     form above and gamma5 D gamma5 D differ by 1 - S^2 = O(delta), so deflation is meant for delta <~ tol.
 
+  * chirally symmetric normal operator (reading G22): A' = 2 + gamma5 S + S gamma5 (normal_op_sym).  Same cost as
+    gamma5 D gamma5 D for a general vector (two signs), ONE sign (sector_op) for a vector of definite chirality -- e.g. a
+    point source in the chiral basis -- and the sector eigenvectors deflate it exactly.
+
 Spinors are canonical arrays [T][Z][Y][X][4][3]; gamma5 = diag(1,1,-1,-1) acts on the spin index (G2).
 """
 from __future__ import annotations
@@ -51,6 +55,21 @@ def sector_op(apply_sign, s: int, x: np.ndarray) -> np.ndarray:
     """A_s x = 2 x + (s + gamma5) sign(H_w) x  for x of chirality s (one application of the sign)."""
     y = apply_sign(x)
     return 2.0 * x + s * y + gamma5(y)
+
+
+def normal_op_sym(apply_sign, x: np.ndarray) -> np.ndarray:
+    """A' x = 2 x + gamma5 S x + S gamma5 x, the chirally symmetric form of D_ov^+ D_ov (reading G22).
+    With S^2 = 1 it IS gamma5 D gamma5 D; with a polynomial sign of error delta the two differ by 1 - S^2 = O(delta), but
+    A' commutes with gamma5 EXACTLY for any Hermitian S and restricted to chirality s it is sector_op: the eigenvectors
+    computed per sector are exact eigenvectors of A' whatever delta is, and a chiral source stays in its sector."""
+    return 2.0 * x + gamma5(apply_sign(x)) + apply_sign(gamma5(x))
+
+
+def chirality_of(x: np.ndarray) -> int:
+    """+1 / -1 if x has a definite chirality (the other half is exactly zero), else 0."""
+    up = np.any(x[..., :2, :] != 0)
+    lo = np.any(x[..., 2:, :] != 0)
+    return +1 if (up and not lo) else (-1 if (lo and not up) else 0)
 
 
 def dense_sign(w: np.ndarray, Zv: np.ndarray) -> np.ndarray:

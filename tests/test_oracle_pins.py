@@ -511,3 +511,32 @@ def test_P17_deflated_multishift_cg_vs_direct_solve(hard4):
         direct = np.linalg.solve(A + s * np.eye(N), b.reshape(-1)).reshape(shape)
         assert rel(x, direct) < 1e-6
     assert it_plain >= 3 * it_defl, (it_plain, it_defl)
+
+
+def test_P18_chirally_symmetric_normal_operator():
+    """A' = 2 + gamma5 S + S gamma5 with a SLOPPY polynomial sign (delta ~ 1e-2): it differs from gamma5 D gamma5 D by
+    exactly 1 - S^2 (so by O(delta)), is Hermitian, commutes with gamma5 to rounding, equals the one-sign sector form on a
+    chiral vector and keeps a chiral vector in its sector -- none of which needs S^2 = 1."""
+    dims = (4, 4, 4, 4)
+    U = wl.su3_links(dims, 0.3, 41)
+    se, n = 0.07, 20
+    coef = ch.cheb_coeffs(n, se * se)
+    assert 1e-3 < ch.delta_measured(coef, se * se) < 0.3
+    with oracle.boundary((1.0, 1.0, 1.0, 1.0)):
+        S = lambda v: oracle.sign_poly(dims, KAPPA, U, coef, se * se, NORM, v)
+        x = wl.gaussian_source(dims, 51)
+        y = wl.gaussian_source(dims, 52)
+        Ax = dfl.normal_op_sym(S, x)
+        dov0 = lambda v: v + dfl.gamma5(S(v))
+        diff = Ax - dfl.normal_op(dov0, x)
+        size = np.linalg.norm(diff.ravel()) / np.linalg.norm(Ax.ravel())
+        assert rel(diff, x - S(S(x))) < 1e-12 and 1e-4 < size < 0.3                # = (1 - S^2) x, visibly non-zero
+        assert rel(dfl.gamma5(Ax), dfl.normal_op_sym(S, dfl.gamma5(x))) < 1e-13    # [A', gamma5] = 0
+        assert abs(vdot(y, Ax) - vdot(dfl.normal_op_sym(S, y), x)) / abs(vdot(y, Ax)) < 1e-13
+        for s in (+1, -1):
+            xs = dfl.chiral_project(x, s)
+            As = dfl.normal_op_sym(S, xs)
+            assert rel(As, dfl.sector_op(S, s, xs)) < 1e-13
+            assert rel(dfl.gamma5(As), s * As) < 1e-13
+            assert dfl.chirality_of(xs) == s
+    assert dfl.chirality_of(x) == 0 and dfl.chirality_of(wl.point_source(dims)) == +1
