@@ -235,6 +235,18 @@ int ov_lanczos_stats(const ov_ctx* ctx, double* out_host);
  *   1 - sign^2 = O(delta)) both <~ tol (mu_j + sigma_i): the defect of w_j enters x_i amplified by 1/(mu_j + sigma_i);
  *   otherwise the true residuals stall near max(delta, resid) |W^+ b| / min(mu + sigma) and relres_out shows it.  Do not combine with ov_set_cg_adaptive
  *   modes 1-2 (an inexact A re-populates the deflated directions).                                                 */
+/* ov_set_cg_operator: which normal operator ov_multishift_cg inverts (reading G22).
+ *   0 (default)  A  = gamma5 D_ov gamma5 D_ov, the plain D_ov^+ D_ov of reading G10: two signs per application;
+ *   1            A' = 2 + gamma5 S + S gamma5, S = the library's sign(H_w).  A' = A + (1 - S^2): the same operator up to
+ *                the polynomial's error delta (they coincide when S^2 = 1), but A' commutes with gamma5 EXACTLY.  So the
+ *                eigenvectors ov_lanczos_dov_lowmodes returns are exact eigenvectors of A' and deflate it whatever delta
+ *                is (no amplification of 1 - S^2 by 1/(mu + sigma)), and for a source of definite chirality (the other
+ *                two spin components exactly zero, e.g. a point source) every CG vector keeps that chirality and one
+ *                application costs ONE sign: half the work.  The solver detects the chirality of the (deflated) source
+ *                itself; ov_cg_chirality returns what the last solve found (+1, -1 or 0).  True residuals are reported
+ *                for A'.  Not combined with the adaptive modes (OV_ESTATE).                                           */
+int ov_set_cg_operator(ov_ctx* ctx, int mode);
+int ov_cg_chirality(const ov_ctx* ctx);
 int ov_lanczos_dov_lowmodes(ov_ctx* ctx, int chirality, int k, double tol, int max_restarts, int cheb_order,
                             int subspace, void* W_out_dev, double* mu_out_host, double* resid_out_host);
 int ov_set_deflation(ov_ctx* ctx, const void* W_dev, const double* mu_host, int k);

@@ -25,7 +25,7 @@ SYMBOLS = [
     "ov_set_dslash_variant", "ov_get_dslash_variant", "ov_pack_spinor", "ov_unpack_spinor", "ov_dslash", "ov_apply_hw",
     "ov_chebyshev_coeffs", "ov_set_polynomial", "ov_set_smallspace", "ov_project", "ov_apply_sign",
     "ov_apply_dov", "ov_apply_dov_reduced", "ov_apply_hw_f32", "ov_set_cg_adaptive", "ov_cg_orders", "ov_apply_hw_host", "ov_apply_dov_host", "ov_blas_axpy", "ov_blas_scale", "ov_blas_dot",
-    "ov_blas_norm2", "ov_multishift_cg", "ov_lanczos_lowmodes", "ov_lanczos_stats", "ov_lanczos_dov_lowmodes", "ov_set_deflation", "ov_host_eigh",
+    "ov_blas_norm2", "ov_multishift_cg", "ov_lanczos_lowmodes", "ov_lanczos_stats", "ov_lanczos_dov_lowmodes", "ov_set_deflation", "ov_set_cg_operator", "ov_cg_chirality", "ov_host_eigh",
 ]
 
 
@@ -329,6 +329,14 @@ class Overlap:
         if rc not in (OV_OK, OV_ENOCONV):
             self._check(rc)
         return W, mu, res, rc == OV_OK
+
+    def set_cg_operator(self, mode):
+        """ov_set_cg_operator: 0 = gamma5 D gamma5 D, 1 = chirally symmetric form (one sign per step for a chiral source)."""
+        self._check(self.lib.ov_set_cg_operator(self._ctx, ctypes.c_int(mode)))
+
+    @property
+    def cg_chirality(self):
+        return int(self.lib.ov_cg_chirality(self._ctx))
 
     def set_deflation(self, W, mu):
         """ov_set_deflation: W [k][12][V] eigenvectors of D_ov^+ D_ov (kept alive here), mu their eigenvalues; None clears."""

@@ -33,6 +33,32 @@ static int apply_A_reduced(ov_ctx* ctx, const double2* in, double2* tmp, double2
     return launch_gamma5(ctx, out, out);
 }
 
+// Chirally symmetric form (ov_set_cg_operator(1); reading G22): out = A' in = 2 in + gamma5 S in + S gamma5 in.
+// A' = gamma5 D gamma5 D + (1 - S^2): the same operator up to the polynomial's error delta, but it commutes with gamma5
+// exactly, so (a) the per-sector eigenvectors of ov_lanczos_dov_lowmodes are its exact eigenvectors whatever delta is and
+// (b) on a vector of definite chirality s it is 2 in + (s + gamma5) S in: ONE sign instead of two.  chir = the chirality of
+// `in` (+-1; the whole Krylov space of a chiral source has it) or 0.  tmp, tmp2: scratch.
+static int apply_A_sym(ov_ctx* ctx, const double2* in, double2* tmp, double2* tmp2, double2* out, int chir) {
+    OV_TRY(apply_sign(ctx, in, tmp));
+    if (chir != 0) return launch_chiral_combine(ctx, 2.0, in, chir, tmp, out);
+    OV_TRY(launch_gamma5(ctx, tmp, tmp));
+    OV_TRY(launch_axpby(ctx, 2.0, in, 1.0, tmp, out));              // out = 2 in + gamma5 S in
+    OV_TRY(launch_gamma5(ctx, in, tmp));
+    OV_TRY(apply_sign(ctx, tmp, tmp2));
+    return launch_axpy(ctx, make_double2(1.0, 0.0), tmp2, out);     // + S gamma5 in
+}
+
+// +1 / -1 if the other chirality half of v is exactly zero, else 0 (tmp: scratch)
+static int chirality_of(ov_ctx* ctx, const double2* v, double2* tmp, int* chir) {
+    double n[2];
+    for (int i = 0; i < 2; i++) {
+        OV_TRY(launch_chiral_combine(ctx, 0.0, nullptr, i == 0 ? +1 : -1, v, tmp));   // 2 P_s v
+        OV_TRY(norm2_host(ctx, tmp, &n[i]));
+    }
+    *chir = (n[1] == 0.0 && n[0] > 0.0) ? +1 : (n[0] == 0.0 && n[1] > 0.0) ? -1 : 0;
+    return OV_OK;
+}
+
 // d[n'] = max over x in [x_lo, 1] of sqrt(x) |P_n(x) - P_n'(x)|: how far the series truncated at n' is from the full
 // polynomial, as an operator on the part of the spectrum the polynomial acts on (host, a few hundred grid points)
 static std::vector<double> truncation_table(const std::vector<double>& c, double eps, double x_lo) {
@@ -59,6 +85,14 @@ static std::vector<double> truncation_table(const std::vector<double>& c, double
 
 using namespace ov;
 
+extern "C" int ov_set_cg_operator(ov_ctx* ctx, int mode) {
+    if (!ctx) return OV_EINVAL;
+    if (mode != 0 && mode != 1) return fail(ctx, OV_EINVAL, "cg operator mode must be 0 or 1");
+    ctx->cg_operator = mode;
+    return OV_OK;
+}
+extern "C" int ov_cg_chirality(const ov_ctx* ctx) { return ctx ? ctx->cg_chirality : 0; }
+
 extern "C" int ov_set_deflation(ov_ctx* ctx, const void* W_dev, const double* mu_host, int k) {
     if (!ctx) return OV_EINVAL;
     if (k < 0 || k > 1024 || (k > 0 && (!W_dev || !mu_host))) return fail(ctx, OV_EINVAL, "bad argument to ov_set_deflation");
@@ -76,6 +110,8 @@ extern "C" int ov_multishift_cg(ov_ctx* ctx, const double* masses_host, int nmas
     if (!masses_host || nmass < 1 || nmass > 64 || !b_ || !x_ || !(tol > 0) || maxiter < 1)
         return fail(ctx, OV_EINVAL, "bad argument to ov_multishift_cg");
     if (ctx->order < 0) return fail(ctx, OV_ESTATE, "ov_set_polynomial has not been called");
+    if (ctx->cg_operator == 1 && ctx->cg_adaptive)
+        return fail(ctx, OV_ESTATE, "the adaptive modes apply to the gamma5 D gamma5 D form only (ov_set_cg_operator(0))");
     const size_t n = spinor_elems(ctx), bytes = n * sizeof(double2);
     ctx->cg_orders.clear();
     const double2* b = (const double2*)b_;
@@ -92,15 +128,21 @@ extern "C" int ov_multishift_cg(ov_ctx* ctx, const double* masses_host, int nmas
     std::sort(ord.begin(), ord.end(), [&](int a, int c) { return sig[a] < sig[c]; });
     const double s0 = sig[ord[0]];
 
-    // device vectors: p_i (nmass), r, q, tmp
+    // device vectors: p_i (nmass), r, q, tmp, tmp2
     double2* pool = nullptr;
-    OV_CUDA(ctx, cudaMalloc(&pool, bytes * (size_t)(nmass + 3)));
+    OV_CUDA(ctx, cudaMalloc(&pool, bytes * (size_t)(nmass + 4)));
     struct Free { double2* p; ~Free() { cudaFree(p); } } guard{pool};
     std::vector<double2*> p(nmass);
     for (int i = 0; i < nmass; i++) p[i] = pool + (size_t)i * n;
     double2* r = pool + (size_t)nmass * n;
     double2* q = r + n;
     double2* tmp = q + n;
+    double2* tmp2 = tmp + n;
+    const bool sym = ctx->cg_operator == 1;
+    int chir = 0;   // symmetric form: chirality of the source (and then of every CG vector), 0 = none
+    auto apply_op = [&](const double2* in, double2* out) -> int {   // the full-accuracy operator of this solve
+        return sym ? apply_A_sym(ctx, in, tmp, tmp2, out, chir) : apply_A(ctx, in, tmp, out);
+    };
 
     double rr;
     OV_TRY(norm2_host(ctx, b, &rr));
@@ -135,6 +177,8 @@ extern "C" int ov_multishift_cg(ov_ctx* ctx, const double* masses_host, int nmas
         OV_TRY(launch_zero(ctx, x + (size_t)i * n));
         OV_TRY(launch_copy(ctx, r, p[i]));
     }
+    if (sym) OV_TRY(chirality_of(ctx, r, tmp, &chir));
+    ctx->cg_chirality = chir;
     // adaptive accuracy (ov_set_cg_adaptive): the application of A at iteration j may be off by eta_j ~ tol |b| / |r_j|
     std::vector<double> trunc;
     if (ctx->cg_adaptive) {
@@ -168,7 +212,8 @@ extern "C" int ov_multishift_cg(ov_ctx* ctx, const double* masses_host, int nmas
             while (order > 1 && 4.0 * trunc[order - 1] <= eta) order--;
             f32 = ctx->cg_adaptive >= 2 && 4.0 * f32_floor <= eta;
         }
-        OV_TRY(apply_A_reduced(ctx, p[0], tmp, q, order, f32));
+        if (sym) OV_TRY(apply_op(p[0], q));
+        else OV_TRY(apply_A_reduced(ctx, p[0], tmp, q, order, f32));
         if (ctx->cg_adaptive) { ctx->cg_orders.push_back(f32 ? -order : order); }
         if (s0 != 0.0) OV_TRY(launch_axpy(ctx, make_double2(s0, 0.0), p[0], q));
         double2 pq;
@@ -222,7 +267,7 @@ extern "C" int ov_multishift_cg(ov_ctx* ctx, const double* masses_host, int nmas
     }
     if (relres_out) {  // true residuals |b - (A + sigma_i) x_i| / |b|
         for (int i = 0; i < nmass; i++) {
-            OV_TRY(apply_A(ctx, x + (size_t)i * n, tmp, q));
+            OV_TRY(apply_op(x + (size_t)i * n, q));
             OV_TRY(launch_axpy(ctx, make_double2(sig[i], 0.0), x + (size_t)i * n, q));
             OV_TRY(launch_axpby(ctx, 1.0, b, -1.0, q, q));
             double e;

@@ -87,6 +87,8 @@ struct ov_ctx {
     std::vector<int> cg_orders;  // order used at each iteration of the last adaptive CG (negative: fp32 sweep)
     std::array<double, 6> lanczos_stats{};  // last ov_lanczos_lowmodes: restarts, filter applies, launches, edge a, widenings, m
     int cg_adaptive = 0;  // ov_set_cg_adaptive: 0 off, 1 reduced orders, 2 reduced orders + fp32 sweeps
+    int cg_operator = 0;  // ov_set_cg_operator: 0 gamma5 D gamma5 D, 1 chirally symmetric form 2 + gamma5 S + S gamma5
+    int cg_chirality = 0; // last solve in the symmetric form: chirality of the source the solver detected (0 = none)
     int flip = 0;  // block order of the next Wilson launch (alternates)
     bool blocked = false;  // layout of spinors and links (see spinor_base)
     long long launches = 0;
