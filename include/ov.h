@@ -179,6 +179,31 @@ int ov_blas_axpy(ov_ctx* ctx, double a_re, double a_im, const void* x, void* y);
 int ov_blas_scale(ov_ctx* ctx, double a, void* x);
 int ov_blas_dot(ov_ctx* ctx, const void* x, const void* y, double* out_host);
 int ov_blas_norm2(ov_ctx* ctx, const void* x, double* out_host);
+/* ov_blas_dot_static: the same scalar product for callers that must not allocate device memory.
+ *   Who that is: ov_blas_dot keeps its per-block partial sums in a buffer its ov_ctx gets from cudaMalloc (at ov_create
+ *   and again, inside the call, when a longer vector needs a bigger one).  An application that has given all of HBM to
+ *   its own pool (eigenvector sets of 17-80 GB leave no slack, so the cudaMalloc fails), or one whose other streams
+ *   must not be stalled by the device-wide synchronisation cudaMalloc/cudaFree imply, cannot use that.  This entry
+ *   point takes no ov_ctx and calls no cudaMalloc, cudaFree or other allocating routine: its partial sums go to a
+ *   fixed 512 KiB array inside libov.so's device image, which every GPU that loads the library holds until the
+ *   process exits.
+ *   Arguments: x_dev, y_dev: n complex128 (re,im) each on the device, read only, may be the same pointer (norm^2);
+ *   out_dev: 2 doubles ON THE DEVICE, receives (re, im) of sum_e conj(x[e]) y[e]; nothing is copied to the host and
+ *   the call does not synchronise -- the result is ready when cuda_stream (a cudaStream_t, NULL = legacy default
+ *   stream) reaches that point.  The GPU owning the buffers and the stream must be the current device.  n = 0 gives 0.
+ *   Limit: n <= ov_blas_dot_static_max() = 33 554 432 (12 components x 2 796 202 sites; 32^3 x 64 fits).  A longer
+ *   vector is rejected with OV_EINVAL before anything is launched.  Other errors: OV_EINVAL (null pointer, n < 0),
+ *   OV_ECUDA.  ov_blas_dot_static_error() returns the message of the calling thread's last failed call.
+ *   Same block shape and summation order as ov_blas_dot: the two agree bit for bit.
+ *   First call on each device: looks up the array's device address (cudaGetSymbolAddress) and caches it; make that
+ *   call before beginning any stream capture.
+ *   Sharing: the one array per GPU serves every call, thread and stream and keeps the previous call's partial sums.
+ *   Each call overwrites the entries it later reads, so no clearing is needed; but two calls that can be in flight on
+ *   the GPU at once (different streams with no event between them) race on it and both results are undefined.
+ *   Calls on one stream are ordered and safe.                                                                      */
+int ov_blas_dot_static(const void* x_dev, const void* y_dev, long long n, void* out_dev, void* cuda_stream);
+long long ov_blas_dot_static_max(void);
+const char* ov_blas_dot_static_error(void);
 
 /* ---- consumers -------------------------------------------------------------------------------------
  * ov_multishift_cg (row a7): solves (A + sigma_i) x_i = b, A = D_ov(0)^+ D_ov(0) applied as

@@ -8,6 +8,8 @@ from .binding import (  # noqa: F401
     SYMBOLS,
     Overlap,
     OvError,
+    blas_dot_static,
+    blas_dot_static_max,
     chebyshev_coeffs,
     host_eigh,
     load_library,

@@ -26,6 +26,7 @@ SYMBOLS = [
     "ov_chebyshev_coeffs", "ov_set_polynomial", "ov_set_smallspace", "ov_project", "ov_apply_sign",
     "ov_apply_dov", "ov_apply_dov_reduced", "ov_apply_hw_f32", "ov_set_cg_adaptive", "ov_cg_orders", "ov_apply_hw_host", "ov_apply_dov_host", "ov_blas_axpy", "ov_blas_scale", "ov_blas_dot",
     "ov_blas_norm2", "ov_multishift_cg", "ov_lanczos_lowmodes", "ov_lanczos_stats", "ov_lanczos_dov_lowmodes", "ov_set_deflation", "ov_set_cg_operator", "ov_cg_chirality", "ov_host_eigh",
+    "ov_blas_dot_static", "ov_blas_dot_static_max", "ov_blas_dot_static_error",
 ]
 
 
@@ -50,6 +51,8 @@ def load_library():
         lib.ov_volume.restype = ctypes.c_longlong
         lib.ov_launch_count.restype = ctypes.c_longlong
         lib.ov_destroy.restype = None
+        lib.ov_blas_dot_static_max.restype = ctypes.c_longlong
+        lib.ov_blas_dot_static_error.restype = ctypes.c_char_p
         _lib = lib
     return _lib
 
@@ -89,6 +92,33 @@ def host_eigh(A: np.ndarray):
     if rc != OV_OK:
         raise OvError(rc, "ov_host_eigh")
     return w, Z
+
+
+def blas_dot_static_max() -> int:
+    """ov_blas_dot_static_max: the longest vector (complex elements) ov_blas_dot_static accepts."""
+    return int(load_library().ov_blas_dot_static_max())
+
+
+def blas_dot_static(x, y, out, stream=None):
+    """ov_blas_dot_static: <x, y> = sum conj(x) y without any device allocation, for programs that cannot call cudaMalloc
+    (all of HBM already in their own pool, or other streams that a cudaMalloc would stall); see include/ov.h.
+
+    x, y: contiguous complex128 CUDA tensors of equal length (any shape); out: a CUDA tensor of 2 float64 (or 1
+    complex128) that the CALLER provides -- this wrapper allocates nothing either -- and that receives (re, im) once
+    `stream` (default: torch's current stream) gets there; nothing is synchronised.  Raises OvError(OV_EINVAL) for more
+    than blas_dot_static_max() elements.  The scratch array behind it is shared per GPU: keep calls on one stream."""
+    if not torch.cuda.is_available():
+        raise OvError(OV_ECUDA, "no CUDA device: this library has no CPU fallback")
+    lib = load_library()
+    assert x.is_cuda and y.is_cuda and out.is_cuda and x.dtype == y.dtype == torch.complex128
+    assert x.numel() == y.numel() and out.numel() * out.element_size() == 16
+    stream = stream if stream is not None else torch.cuda.current_stream(x.device)
+    with torch.cuda.device(x.device):
+        rc = lib.ov_blas_dot_static(_ptr(x), _ptr(y), ctypes.c_longlong(x.numel()), _ptr(out),
+                                    ctypes.c_void_p(stream.cuda_stream))
+    if rc != OV_OK:
+        raise OvError(rc, lib.ov_blas_dot_static_error().decode())
+    return out
 
 
 class OvOptions(ctypes.Structure):
