@@ -274,14 +274,38 @@ def algorithmic_bytes_per_sign(order, V, with_low, recon=18):
     return total * V
 
 
+def modes_residual(op, V, lam, norm):
+    """max_i |Q v_i - lambda_i v_i|, Q = H_w/norm, recomputed with the context's own kernels."""
+    worst = 0.0
+    for i in range(V.shape[0]):
+        r = op.apply_hw(V[i])
+        op.blas_scale(1.0 / norm, r)
+        op.blas_axpy(-float(lam[i]), V[i], r)
+        worst = max(worst, float(np.sqrt(op.blas_norm2(r))))
+    return worst
+
+
 def get_low_modes(op, cfg, k, args, log):
+    """The k low modes of Q: from --modes-file when it fits this context, else from the library's Lanczos.  The file holds
+    V in the context's ABI layout, so it records that layout (ov_spinor_layout) beside the dims; a file written under
+    another layout (or without the key) is not used.  The residuals of loaded modes are recomputed, never taken from
+    the file."""
     import torch
     path = args.modes_file
     if path and os.path.exists(path):
         d = torch.load(path, map_location="cpu", weights_only=True)
-        if d["V"].shape[0] >= k and tuple(d["dims"].tolist()) == tuple(cfg.dims):
-            log(f"low modes: loaded {path}")
-            return d["V"][:k].cuda().contiguous(), d["lam"][:k].numpy(), float(d["resid"]), 0.0
+        same_dims = tuple(d["dims"].tolist()) == tuple(cfg.dims)
+        same_layout = "layout" in d and int(d["layout"]) == op.spinor_layout
+        if d["V"].shape[0] >= k and same_dims and same_layout:
+            V, lam = d["V"][:k].cuda().contiguous(), d["lam"][:k].numpy()
+            resid = modes_residual(op, V, lam, cfg.norm)
+            if resid <= 1e-8:
+                log(f"low modes: loaded {path} (layout {op.spinor_layout}, residual recomputed: {resid:.2e})")
+                return V, lam, resid, 0.0
+            log(f"low modes: {path} rejected, recomputed residual {resid:.2e} > 1e-8 (other gauge field or norm?)")
+        else:
+            log(f"low modes: {path} not usable here (k, dims or spinor layout differ: this context has layout "
+                f"{op.spinor_layout}); running Lanczos")
     t0 = time.perf_counter()
     V, lam, res, ok = op.lanczos_lowmodes(k, tol=1e-8, max_restarts=60, cheb_order=args.lanczos_order)
     torch.cuda.synchronize()
@@ -292,7 +316,7 @@ def get_low_modes(op, cfg, k, args, log):
         raise RuntimeError(f"Lanczos did not reach 1e-8 (max residual {res.max():.2e})")
     if path:
         torch.save({"V": V.cpu(), "lam": torch.from_numpy(lam), "resid": torch.tensor(float(res.max())),
-                    "dims": torch.tensor(cfg.dims)}, path)
+                    "dims": torch.tensor(cfg.dims), "layout": torch.tensor(op.spinor_layout)}, path)
     return V, lam, float(res.max()), dt
 
 
@@ -382,7 +406,7 @@ def run_b200(args):
         ne2e = min(4, nsrc)
         hin = torch.stack([h for h in host_src[:ne2e]]).contiguous().pin_memory()
         hout = torch.empty_like(hin).pin_memory()
-        nst = max(2, min(args.steps, 3))
+        nst = max(2, min(args.steps, 8))
         ms_e = timed(lambda i: op.apply_dov_host(0.0, hin, hout), 1, nst)
         nbytes = hin.numel() * 16
         e2e = {"value": aggregate_value(world, nst * ne2e, ms_e), "unit": UNIT, "h2d_bytes_per_step": nbytes,
@@ -455,7 +479,10 @@ def run_b200(args):
         torch.cuda.synchronize()
         cg["symmetric"] = {"seconds": time.perf_counter() - t0, "iterations": iters, "converged": bool(okc),
                            "chirality_detected": op.cg_chirality,
-                           "note": "A' = 2 + gamma5 S + S gamma5 (= gamma5 D gamma5 D up to 1 - S^2): one sign per application for a chiral source"}
+                           "note": "a DIFFERENT operator from 'plain': A' = 2 + gamma5 S + S gamma5 = gamma5 D gamma5 D + (1 - S^2), i.e. O(delta) away from "
+                                   "the D_ov^+ D_ov of reading G10 (DESIGN.md reading G22, the builder's option, not the paper's); "
+                                   "one sign per application holds for chiral sources only (the point source here is one). "
+                                   "Not a speed-up of the 'plain' solve"}
         op.set_cg_operator(0)
         del xs, bsrc
     # ---- deflated multi-mass CG on the workload built for it, reported separately
