@@ -24,9 +24,11 @@
  *   canonical gauge   complex128 [T][Z][Y][X][mu][row][col]   U_mu(x) links x -> x+mu
  *   canonical spinor  complex128 [T][Z][Y][X][spin][colour]   (= [site][12])
  *   ABI spinor        12*V complex128, site-major SoA in one of two forms, fixed per context (ov_spinor_layout):
- *                       1 "blocked" (whenever V is a multiple of 32): component q = 3*spin+colour of site i at complex
+ *                       1 "blocked" (needs V % 32 == 0): component q = 3*spin+colour of site i at complex
  *                         index ((i/32)*12 + q)*32 + i%32   -- 32-site blocks, components of a block contiguous;
- *                       0 "planes" (any other V): component q of site i at q*V + i.
+ *                       0 "planes" (any V): component q of site i at q*V + i.
+ *                     Which one a context uses is decided at ov_create_ex (ov_options.layout; the automatic rule is
+ *                     stated there: planes where the TMA-staged Wilson kernel applies, else blocked when V % 32 == 0).
  *                     (re,im) interleaved; nrhs vectors are consecutive (stride 12*V).  Callers normally never index
  *                     it: ov_pack_spinor / ov_unpack_spinor convert canonical <-> ABI on the device, and every
  *                     BLAS-1 / projector entry point is layout-agnostic.
@@ -65,6 +67,10 @@ int ov_create(ov_ctx** out, const int dims[4], double kappa, const void* gauge_d
 /* ov_create_ex: the same with options (NULL or all-zero = ov_create).
  *   layout      0 automatic (planes when the TMA-staged Wilson kernel applies, i.e. X % 8 == 0, Y % 4 == 0, Z % 4 == 0;
  *                 else blocked when V % 32 == 0; else planes), 1 blocked (needs V % 32 == 0), 2 planes.
+ *                 "Applies" is checked, not assumed: ov_create_ex builds the tensor maps of the gauge field once; if
+ *                 the driver's cuTensorMapEncodeTiled is missing or refuses them, or the environment variable OV_NO_TMA
+ *                 is set (to anything but "0"), the context behaves as on a lattice where the kernel does not apply
+ *                 (automatic layout -> blocked when V % 32 == 0, automatic variant -> gather, variant 2 -> OV_EINVAL).
  *   t_boundary  what the hop between t = T-1 and t = 0 is multiplied by: OV_BC_ANTIPERIODIC (-1, the default of this
  *               library: north_star, reading G11), OV_BC_PERIODIC (+1), OV_BC_OPEN (0: no hop across the
  *               boundary, the Dirichlet condition in time of PAPER.md:104).
@@ -258,8 +264,11 @@ int ov_lanczos_stats(const ov_ctx* ctx, double* out_host);
  *   eigenvectors of the operator the CG applies (gamma5 D_ov gamma5 D_ov with the current polynomial) to within tol,
  *   i.e. eigensolver residual and polynomial error delta (the sector form differs from gamma5 D gamma5 D by
  *   1 - sign^2 = O(delta)) both <~ tol (mu_j + sigma_i): the defect of w_j enters x_i amplified by 1/(mu_j + sigma_i);
- *   otherwise the true residuals stall near max(delta, resid) |W^+ b| / min(mu + sigma) and relres_out shows it.  Do not combine with ov_set_cg_adaptive
- *   modes 1-2 (an inexact A re-populates the deflated directions).                                                 */
+ *   otherwise the true residuals stall near max(delta, resid) |W^+ b| / min(mu + sigma) and relres_out shows it.
+ *   Enforced: with a deflation space set, ov_multishift_cg returns OV_ESTATE under ov_set_cg_adaptive modes 1-2 (an
+ *   inexact A re-populates the deflated directions) and OV_EINVAL if some mu_j + sigma_i <= 0 (a zero mode with mass 0:
+ *   the shifted system is singular); ov_set_polynomial and ov_set_smallspace change the operator the w_j belong to and
+ *   therefore CLEAR the deflation space (call ov_set_deflation again with eigenpairs of the new operator).          */
 /* ov_set_cg_operator: which normal operator ov_multishift_cg inverts (reading G22).
  *   0 (default)  A  = gamma5 D_ov gamma5 D_ov, the plain D_ov^+ D_ov of reading G10: two signs per application;
  *   1            A' = 2 + gamma5 S + S gamma5, S = the library's sign(H_w).  A' = A + (1 - S^2): the same operator up to

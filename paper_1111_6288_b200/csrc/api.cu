@@ -57,7 +57,7 @@ int ensure_reduction_buffers(ov_ctx* ctx, size_t partial_elems, size_t result_el
     return OV_OK;
 }
 
-static bool tma_usable(const ov_ctx* ctx) { return !ctx->blocked && tma_eligible(ctx->lat); }
+static bool tma_usable(const ov_ctx* ctx) { return ctx->tma_ok && !ctx->blocked && tma_eligible(ctx->lat); }
 
 int effective_variant(const ov_ctx* ctx) {
     if (ctx->dslash_variant == 1) return 1;
@@ -150,6 +150,13 @@ int ov_create_ex(ov_ctx** out, const int dims[4], double kappa, const void* gaug
     const size_t gbytes = gauge_elems(ctx->lat.V, recon) * sizeof(double2);
     cudaError_t e = cudaMalloc(&ctx->gauge, gbytes);
     if (e != cudaSuccess) { delete ctx; return e == cudaErrorMemoryAllocation ? OV_ENOMEM : OV_ECUDA; }
+    // the planes layout was chosen for the TMA-staged kernel: make sure tensor maps can actually be built here, and if
+    // not (driver entry point missing, encode refused, OV_NO_TMA) fall back NOW, while the layout can still change, to
+    // what a non-eligible lattice gets -- the gather kernel on the blocked layout -- instead of failing at every launch
+    if (!ctx->blocked && tma_eligible(ctx->lat) && !tma_probe(ctx)) {
+        ctx->tma_ok = false;
+        if (opt.layout == 0 && ctx->lat.V % 32 == 0) ctx->blocked = true;
+    }
     int rc = OV_OK;
     if (recon == 12) {   // rows 0-1 only make sense if row 2 really is conj(row0 x row1)
         double defect = 0.0;

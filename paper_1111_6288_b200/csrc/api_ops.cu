@@ -42,6 +42,13 @@ int ov_chebyshev_coeffs(int order, double eps, double* coeffs_host) {
     return OV_OK;
 }
 
+// the deflation space holds eigenpairs of D_ov^+ D_ov for the sign function in force when they were computed: a new
+// polynomial or small space changes that operator, so the (borrowed) space is dropped rather than left to go stale
+static void drop_deflation(ov_ctx* ctx) {
+    ctx->Wdefl = nullptr;
+    ctx->mu_defl.clear();
+}
+
 int ov_set_polynomial(ov_ctx* ctx, const double* coeffs_host, int order, double eps, double norm) {
     if (!ctx) return OV_EINVAL;
     if (!coeffs_host || order < 0) return fail(ctx, OV_EINVAL, "null coefficients or negative order");
@@ -49,6 +56,7 @@ int ov_set_polynomial(ov_ctx* ctx, const double* coeffs_host, int order, double 
     if (!(norm > 0.0)) return fail(ctx, OV_EINVAL, "norm must be positive");
     for (int j = 0; j <= order; j++)
         if (!std::isfinite(coeffs_host[j])) return fail(ctx, OV_EINVAL, "coefficient %d is not finite", j);
+    drop_deflation(ctx);
     ctx->coef.assign(coeffs_host, coeffs_host + order + 1);
     ctx->order = order;
     ctx->eps = eps;
@@ -59,7 +67,7 @@ int ov_set_polynomial(ov_ctx* ctx, const double* coeffs_host, int order, double 
 int ov_set_smallspace(ov_ctx* ctx, const void* V_dev, const double* lambda_host, int k) {
     if (!ctx) return OV_EINVAL;
     if (k < 0) return fail(ctx, OV_EINVAL, "k < 0");
-    if (k == 0) { ctx->k = 0; ctx->Vlow = nullptr; ctx->lambda.clear(); return OV_OK; }
+    if (k == 0) { ctx->k = 0; ctx->Vlow = nullptr; ctx->lambda.clear(); drop_deflation(ctx); return OV_OK; }
     if (!V_dev || !lambda_host) return fail(ctx, OV_EINVAL, "null V or lambda with k > 0");
     if ((size_t)k * 2 * sizeof(double2) > 200 * 1024) return fail(ctx, OV_EINVAL, "k too large (max 6400)");
     std::vector<double> sgn(k);
@@ -81,6 +89,7 @@ int ov_set_smallspace(ov_ctx* ctx, const void* V_dev, const double* lambda_host,
     ctx->Vlow = (const double2*)V_dev;
     ctx->lambda.assign(lambda_host, lambda_host + k);
     ctx->k = k;
+    drop_deflation(ctx);
     return OV_OK;
 }
 
@@ -159,27 +168,53 @@ int ov_cg_orders(const ov_ctx* ctx, int* out_host, int cap) {
 // host-buffer path: H2D -> pack -> operator -> unpack -> D2H.  With nrhs > 1 the copies run on two copy streams (one per
 // direction, double-buffered canonical staging): the H2D of right-hand side r+1 and the D2H of r-1 overlap the operator on r,
 // so only the first H2D and the last D2H are exposed.  Host buffers should be pinned for the copies to be asynchronous.
+// Staging of the host-buffer path.  Every member is created only if it is still null, so a call that failed half way
+// (an allocation that did not fit, say) leaves a state the next call completes instead of overwriting -- nothing leaks,
+// and ov_destroy frees whatever exists.  nbuf = 1 (a single right-hand side: nothing to overlap) creates one staging
+// buffer and one event set per direction, nbuf = 2 the double-buffered set: 4 resp. 6 spinors of device memory.
+static int host_pipe_prepare(ov_ctx* ctx, int nbuf) {
+    HostPipe& hp = ctx->host_pipe;
+    const size_t bytes = spinor_elems(ctx) * sizeof(double2);
+    auto buffer = [&](double2** p) -> int {
+        if (*p) return OV_OK;
+        const cudaError_t e = cudaMalloc(p, bytes);
+        if (e != cudaSuccess) { *p = nullptr; cudaGetLastError(); return cuda_fail(ctx, e, "cudaMalloc (host-path staging)"); }
+        return OV_OK;
+    };
+    auto event = [&](cudaEvent_t* ev) -> int {
+        if (*ev) return OV_OK;
+        const cudaError_t e = cudaEventCreateWithFlags(ev, cudaEventDisableTiming);
+        if (e != cudaSuccess) { *ev = nullptr; return cuda_fail(ctx, e, "cudaEventCreateWithFlags (host path)"); }
+        return OV_OK;
+    };
+    auto stream = [&](cudaStream_t* st) -> int {
+        if (*st) return OV_OK;
+        const cudaError_t e = cudaStreamCreateWithFlags(st, cudaStreamNonBlocking);
+        if (e != cudaSuccess) { *st = nullptr; return cuda_fail(ctx, e, "cudaStreamCreateWithFlags (host path)"); }
+        return OV_OK;
+    };
+    for (int b = 0; b < nbuf; b++) {
+        OV_TRY(buffer(&hp.cin[b]));
+        OV_TRY(buffer(&hp.cout[b]));
+        OV_TRY(event(&hp.in_ready[b]));
+        OV_TRY(event(&hp.in_free[b]));
+        OV_TRY(event(&hp.out_ready[b]));
+        OV_TRY(event(&hp.out_free[b]));
+    }
+    OV_TRY(buffer(&hp.abi_in));
+    OV_TRY(buffer(&hp.abi_out));
+    OV_TRY(stream(&hp.h2d));
+    OV_TRY(stream(&hp.d2h));
+    OV_TRY(event(&hp.start));
+    return OV_OK;
+}
+
 static int host_apply(ov_ctx* ctx, int which, double mass, const void* in_host, void* out_host, int nrhs) {
     if (!ctx) return OV_EINVAL;
     if (!in_host || !out_host || nrhs < 1) return fail(ctx, OV_EINVAL, "null pointer or nrhs < 1");
     const size_t n = spinor_elems(ctx), bytes = n * sizeof(double2);
     HostPipe& hp = ctx->host_pipe;
-    if (!hp.ready) {
-        for (int b = 0; b < 2; b++) {
-            OV_CUDA(ctx, cudaMalloc(&hp.cin[b], bytes));
-            OV_CUDA(ctx, cudaMalloc(&hp.cout[b], bytes));
-            OV_CUDA(ctx, cudaEventCreateWithFlags(&hp.in_ready[b], cudaEventDisableTiming));
-            OV_CUDA(ctx, cudaEventCreateWithFlags(&hp.in_free[b], cudaEventDisableTiming));
-            OV_CUDA(ctx, cudaEventCreateWithFlags(&hp.out_ready[b], cudaEventDisableTiming));
-            OV_CUDA(ctx, cudaEventCreateWithFlags(&hp.out_free[b], cudaEventDisableTiming));
-        }
-        OV_CUDA(ctx, cudaMalloc(&hp.abi_in, bytes));
-        OV_CUDA(ctx, cudaMalloc(&hp.abi_out, bytes));
-        OV_CUDA(ctx, cudaStreamCreateWithFlags(&hp.h2d, cudaStreamNonBlocking));
-        OV_CUDA(ctx, cudaStreamCreateWithFlags(&hp.d2h, cudaStreamNonBlocking));
-        OV_CUDA(ctx, cudaEventCreateWithFlags(&hp.start, cudaEventDisableTiming));
-        hp.ready = true;
-    }
+    OV_TRY(host_pipe_prepare(ctx, nrhs > 1 ? 2 : 1));
     // the copy streams start after everything the caller enqueued on the context's stream so far
     OV_CUDA(ctx, cudaEventRecord(hp.start, ctx->stream));
     OV_CUDA(ctx, cudaStreamWaitEvent(hp.h2d, hp.start, 0));

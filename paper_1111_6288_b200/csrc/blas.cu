@@ -430,13 +430,20 @@ int launch_multi_dot(ov_ctx* ctx, const double2* xs, size_t stride, int nvec, co
     return launch_multi_dot_at(ctx, xs, stride, nvec, y, 0, nvec);
 }
 
+// the batched kernel parks all nb * nvec per-warp sums of a block in shared memory (128 B per result): nb = 4 fits up to
+// nvec = 400, nb = 2 up to 800; callers (project_batch) take smaller groups beyond that
+bool multi_dot_batch_fits(int nvec, int nb) {
+    return (size_t)nb * nvec * kDotWarps * sizeof(double2) <= 200 * 1024;
+}
+
 // nb in {2, 4} right-hand sides y_r = y + r * ystride in one pass over the x_j: d_result[r * nvec + j] = <x_j, y_r>
 int launch_multi_dot_batch(ov_ctx* ctx, const double2* xs, size_t stride, int nvec, const double2* y, size_t ystride, int nb) {
     const long long n = (long long)spinor_elems(ctx);
     const long long nblocks = (n + kDotBlockElems - 1) / kDotBlockElems;
     if (nb != 2 && nb != 4) return fail(ctx, OV_EINVAL, "multi_dot_batch: nb must be 2 or 4");
     const size_t shmem = (size_t)nb * nvec * kDotWarps * sizeof(double2);
-    if (shmem > 200 * 1024) return fail(ctx, OV_EINVAL, "multi_dot_batch: %d x %d results do not fit in shared memory", nb, nvec);
+    if (!multi_dot_batch_fits(nvec, nb))
+        return fail(ctx, OV_EINVAL, "multi_dot_batch: %d x %d results do not fit in shared memory", nb, nvec);
     OV_TRY(ensure_reduction_buffers(ctx, (size_t)nblocks * nb * nvec, (size_t)nb * nvec));
     if (nb == 2) {
         if (shmem > 48 * 1024)

@@ -112,6 +112,9 @@ extern "C" int ov_multishift_cg(ov_ctx* ctx, const double* masses_host, int nmas
     if (ctx->order < 0) return fail(ctx, OV_ESTATE, "ov_set_polynomial has not been called");
     if (ctx->cg_operator == 1 && ctx->cg_adaptive)
         return fail(ctx, OV_ESTATE, "the adaptive modes apply to the gamma5 D gamma5 D form only (ov_set_cg_operator(0))");
+    if (!ctx->mu_defl.empty() && ctx->cg_adaptive)
+        return fail(ctx, OV_ESTATE, "deflation (ov_set_deflation) and the adaptive modes (ov_set_cg_adaptive) cannot be combined: "
+                                    "an inexact operator re-populates the deflated directions");
     const size_t n = spinor_elems(ctx), bytes = n * sizeof(double2);
     ctx->cg_orders.clear();
     const double2* b = (const double2*)b_;
@@ -123,6 +126,13 @@ extern "C" int ov_multishift_cg(ov_ctx* ctx, const double* masses_host, int nmas
         if (!(m * m < 4.0)) return fail(ctx, OV_EINVAL, "mass %d out of range", i);
         sig[i] = m * m / (1.0 - 0.25 * m * m);
     }
+    // the deflated part of x_i divides by mu_j + sigma_i: a zero mode (or rounding noise below zero, which ov_set_deflation
+    // lets through) with mass 0 would make the system singular
+    for (size_t j = 0; j < ctx->mu_defl.size(); j++)
+        for (int i = 0; i < nmass; i++)
+            if (!(ctx->mu_defl[j] + sig[i] > 0.0))
+                return fail(ctx, OV_EINVAL, "deflation mode %zu (mu = %g) with mass %d (sigma = %g): mu + sigma <= 0, the shifted system is singular",
+                            j, ctx->mu_defl[j], i, sig[i]);
     std::vector<int> ord(nmass);
     std::iota(ord.begin(), ord.end(), 0);
     std::sort(ord.begin(), ord.end(), [&](int a, int c) { return sig[a] < sig[c]; });

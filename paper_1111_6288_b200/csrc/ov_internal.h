@@ -60,8 +60,7 @@ using EpilogueF = EpilogueT<float2>;
 }  // namespace ov
 
 // staging of the *_host entry points (api_ops.cu::host_apply)
-struct HostPipe {
-    bool ready = false;
+struct HostPipe {   // members are created on demand by api_ops.cu::host_pipe_prepare (null = not created yet)
     double2* cin[2] = {nullptr, nullptr};    // canonical input, double-buffered
     double2* cout[2] = {nullptr, nullptr};   // canonical output, double-buffered
     double2* abi_in = nullptr;
@@ -84,6 +83,7 @@ struct ov_ctx {
     double field_qE = 0.0;     // it; the Wilson kernels need it only to rebuild the third row of 12-real t links
     int field_origin = 0;
     void* tma_state = nullptr; // tensor maps and schedule of the TMA-staged kernel (wilson_tma.cu)
+    bool tma_ok = true;        // false: tma_probe failed at ov_create_ex, the context never picks the TMA-staged kernel
     std::vector<int> cg_orders;  // order used at each iteration of the last adaptive CG (negative: fp32 sweep)
     std::array<double, 6> lanczos_stats{};  // last ov_lanczos_lowmodes: restarts, filter applies, launches, edge a, widenings, m
     int cg_adaptive = 0;  // ov_set_cg_adaptive: 0 off, 1 reduced orders, 2 reduced orders + fp32 sweeps
@@ -173,6 +173,7 @@ int effective_variant(const ov_ctx* ctx);  // 1 = gather, 2 = TMA-staged: what l
 int launch_wilson_gather(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep);
 int launch_wilson_tma(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep);   // variant 2 (wilson_tma.cu)
 bool tma_eligible(const Lattice& lat);
+bool tma_probe(const ov_ctx* ctx);   // tensor maps can be built for this context (needs ctx->gauge allocated); see wilson_tma.cu
 void tma_state_free(ov_ctx* ctx);
 // batched: nrhs consecutive ABI spinors (stride 12 V) in in/out and in every epilogue operand
 int launch_wilson_batch(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep, int nrhs);
@@ -219,6 +220,7 @@ int ensure_gauge_f32(ov_ctx* ctx);
 int workspace_f32(ov_ctx* ctx, int i, float2** out);
 
 int launch_multi_dot_batch(ov_ctx* ctx, const double2* xs, size_t stride, int nvec, const double2* y, size_t ystride, int nb);
+bool multi_dot_batch_fits(int nvec, int nb);   // does the nb x nvec result block of launch_multi_dot_batch fit in shared memory
 // projector: c = V^+ x (left in ctx->d_result[0..k)); perp = x - V c; low = V (sgn o c)
 int project(ov_ctx* ctx, const double2* x, double2* perp, double2* low);
 // the same for nb consecutive right-hand sides (stride 12 V) with V streamed once per pass for groups of 4 / 2 of them

@@ -55,7 +55,9 @@ int project_batch(ov_ctx* ctx, const double2* x, double2* perp, double2* low, in
     const size_t stride = spinor_elems(ctx);
     int r0 = 0;
     while (r0 < nb) {
-        const int g = (nb - r0 >= 4) ? 4 : (nb - r0 >= 2) ? 2 : 1;
+        // group of 4 or 2 where the batched dot's result block fits in shared memory (k <= 400 / 800), else one at a time
+        const int g = (nb - r0 >= 4 && multi_dot_batch_fits(ctx->k, 4)) ? 4
+                    : (nb - r0 >= 2 && multi_dot_batch_fits(ctx->k, 2)) ? 2 : 1;
         if (g == 1) {
             OV_TRY(project(ctx, x + r0 * stride, perp + r0 * stride, low + r0 * stride));
         } else {

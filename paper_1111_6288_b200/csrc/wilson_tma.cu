@@ -27,6 +27,7 @@
 // Needs the planes layout and X % 8 == 0, Y % 4 == 0, Z % 4 == 0; other shapes use the gather kernel.
 #include <cuda.h>
 
+#include <cstdlib>
 #include <unordered_map>
 
 #include "ov_internal.h"
@@ -562,6 +563,19 @@ bool tma_eligible(const Lattice& lat) {
            lat.Z <= 256;
 }
 
+// Can this context use the TMA-staged kernel at all?  Asked once, at ov_create_ex, before the layout is fixed: the driver
+// entry point cuTensorMapEncodeTiled must resolve and must accept the tensor maps of this lattice (tried on the gauge
+// array; only the pointer is used).  The environment variable OV_NO_TMA (set, not "0") answers no: a switch for drivers
+// or tools that mishandle tensor maps, and the test hook for the fallback.
+bool tma_probe(const ov_ctx* ctx) {
+    const char* off = std::getenv("OV_NO_TMA");
+    if (off && off[0] && !(off[0] == '0' && !off[1])) return false;
+    if (!tma_eligible(ctx->lat) || !encode_fn()) return false;
+    Maps m;
+    const int NE = ctx->recon / 2;
+    return make_maps(&m, ctx->gauge, ctx->lat, 4 * NE, NE);
+}
+
 void tma_state_free(ov_ctx* ctx) {
     delete (TmaState*)ctx->tma_state;
     ctx->tma_state = nullptr;
@@ -569,11 +583,16 @@ void tma_state_free(ov_ctx* ctx) {
 
 template <int RECON, int NA>
 static cudaError_t launch_k(const Args& a, int grid, size_t smem, cudaStream_t st) {
-    static bool attr_set = false;   // per instantiation; one device per process (bench.py: one process per GPU)
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(wilson_tma_kernel<RECON, NA>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    // the opt-in to > 48 KB of dynamic shared memory is a per-device property of the function: remember it per
+    // instantiation AND per device ordinal (a process may hold contexts on several GPUs); beyond 64 devices set it each time
+    static bool attr_set[64] = {};
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64 || !attr_set[dev]) {
+        e = cudaFuncSetAttribute(wilson_tma_kernel<RECON, NA>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        attr_set = true;
+        if (dev >= 0 && dev < 64) attr_set[dev] = true;
     }
     wilson_tma_kernel<RECON, NA><<<grid, Form<NA>::threads, smem, st>>>(a);
     return cudaGetLastError();

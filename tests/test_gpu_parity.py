@@ -353,6 +353,28 @@ def test_batched_apply_matches_single_and_oracle(ovp, cfg0, with_small):
     assert rel(got_d[6], ref) <= TOL_DOV
 
 
+@pytest.mark.parametrize("k", [401, 801])
+def test_batched_projector_with_many_modes(ovp, cfg0, k):
+    """The batched V^+ x keeps 128 B of shared memory per (mode, rhs): groups of 4 fit up to k = 400, groups of 2 up to 800.
+    Beyond that the batch must fall back to smaller groups (k = 401: pairs; k = 801: one at a time) instead of failing,
+    with the per-rhs result unchanged.  V: any orthonormal set does for the projector algebra (QR of a Gaussian matrix)."""
+    cfg = cfg0["cfg"]
+    rng = np.random.default_rng(k)
+    n = 12 * wl.volume(cfg.dims)
+    Qm, _ = np.linalg.qr(rng.standard_normal((n, k)) + 1j * rng.standard_normal((n, k)))
+    V = np.ascontiguousarray(Qm.T).reshape((k,) + cfg0["x"].shape)
+    lam = rng.uniform(0.01, 0.05, k) * rng.choice([-1.0, 1.0], k)
+    op = make(ovp, cfg.dims, cfg0["U"])
+    op.set_polynomial(ovp.chebyshev_coeffs(4, cfg.eps), cfg.eps, cfg.norm)
+    op.set_smallspace(to_dev(op, V), lam)
+    xs = np.stack([wl.gaussian_source(cfg.dims, 70 + j) for j in range(5)])    # a group of 4 and a single
+    got = to_host(op, op.apply_sign(to_dev(op, xs)))
+    for j in range(len(xs)):
+        assert np.array_equal(got[j], to_host(op, op.apply_sign(to_dev(op, xs[j]))))
+    # the low part is exact on span(V): sign(v_0) = sign(lam_0) v_0 up to the polynomial acting on rounding noise
+    assert rel(to_host(op, op.apply_sign(to_dev(op, V[0]))), np.sign(lam[0]) * V[0]) <= 1e-12
+
+
 def test_timing_hooks_and_launch_count(ovp, cfg0):
     """bench.py's roofline reads these: every launch inside the Clenshaw sweep is the Wilson kernel (2n+1 per sign)."""
     op, _ = setup_op(ovp, cfg0)
@@ -407,6 +429,30 @@ def test_tma_variant_sign_and_dov_vs_oracle(ovp, recon):
 
 
 # ------------------------------------------------------------------------------------------ links that are not SU(3)
+def test_fallback_when_tensor_maps_are_unavailable(ovp, monkeypatch):
+    """If tensor maps cannot be built (driver entry point missing, encode refused -- forced here with OV_NO_TMA), a context
+    in automatic mode must not fail at every Wilson launch: it falls back at ov_create_ex to what a non-eligible lattice
+    gets (blocked layout, gather kernel), still matches the oracle, and refuses an explicit variant 2."""
+    dims = (8, 4, 4, 6)
+    U = wl.su3_links(dims, 0.5, 5)
+    x = wl.gaussian_source(dims, 6)
+    ref = oracle.hw(dims, KAPPA, U, x)
+    op = make(ovp, dims, U)
+    assert op.dslash_variant == 2 and op.spinor_layout == 0
+    assert rel(to_host(op, op.apply_hw(to_dev(op, x))), ref) <= TOL_HW
+    monkeypatch.setenv("OV_NO_TMA", "1")
+    op = make(ovp, dims, U)
+    assert op.dslash_variant == 1 and op.spinor_layout == 1
+    assert rel(to_host(op, op.apply_hw(to_dev(op, x))), ref) <= TOL_HW
+    with pytest.raises(ovp.OvError):
+        op.set_dslash_variant(2)
+    op = ovp.Overlap(dims, KAPPA, U, layout="planes")          # explicit planes layout: kept, but the gather kernel runs
+    assert op.dslash_variant == 1 and op.spinor_layout == 0
+    assert rel(to_host(op, op.apply_hw(to_dev(op, x))), ref) <= TOL_HW
+    monkeypatch.setenv("OV_NO_TMA", "0")                        # "0" does not switch it off
+    assert make(ovp, dims, U).dslash_variant == 2
+
+
 def test_u3_and_dirichlet_links(ovp):
     """recon 18 takes any 3x3 links: a U(1) background phase on every link (U -> e^{-iqA} U) and zero links
     across a Dirichlet boundary in x and t; recon 12 must refuse them (row 2 could not be rebuilt)."""
@@ -588,6 +634,26 @@ def test_deflation_degenerate_inputs(ovp):
     bh, xh = to_host(op, b), to_host(op, x)
     for i, m in enumerate(masses):
         assert rel(xh[i], bh / (mu[1] + sigma_of_mass(m))) <= 1e-8
+    # preconditions the solver enforces (include/ov.h, ov_set_deflation): no adaptive modes with a deflation space ...
+    op.set_cg_adaptive(1)
+    with pytest.raises(ovp.OvError) as ei:
+        op.multishift_cg(masses, b, tol=1e-8, maxiter=100)
+    assert ei.value.code == ovp.binding.OV_ESTATE
+    op.set_cg_adaptive(0)
+    # ... and no mu_j + sigma_i <= 0: a zero mode with mass 0 would be divided by zero
+    op.set_deflation(W, np.array([0.0, mu[1], mu[2]]))
+    with pytest.raises(ovp.OvError) as ei:
+        op.multishift_cg((0.0, 0.1), b, tol=1e-8, maxiter=100)
+    assert ei.value.code == ovp.binding.OV_EINVAL and "singular" in str(ei.value)
+    x0, it0, rr0, ok0 = op.multishift_cg(masses, b, tol=1e-8, maxiter=100)     # the same space with masses > 0 is fine
+    assert ok0 and it0 == 0 and np.all(np.isfinite(to_host(op, x0)))
+    # a new polynomial (or small space) changes the operator: the deflation space is dropped, not left stale
+    op.set_deflation(W, mu)
+    op.set_polynomial(ovp.chebyshev_coeffs(n, se * se), se * se, NORM)
+    _, iters1, relres1, ok1 = op.multishift_cg(masses, b, tol=1e-8, maxiter=500)
+    assert ok1 and iters1 > 0 and np.all(relres1 <= 1e-8)
+    op.set_deflation(W, mu)
+    assert op.multishift_cg(masses, b, tol=1e-8, maxiter=100)[1] == 0
     op.set_deflation(None, None)
     _, iters2, relres2, ok2 = op.multishift_cg(masses, b, tol=1e-8, maxiter=500)
     assert ok2 and iters2 > 0 and np.all(relres2 <= 1e-8)
