@@ -312,6 +312,10 @@ def get_low_modes(op, cfg, k, args, log):
     dt = time.perf_counter() - t0
     log(f"low modes: Lanczos k={k} in {dt:.1f} s, max residual {res.max():.2e}, converged={ok}, "
         f"|lambda| in [{np.abs(lam).min():.5f}, {np.abs(lam).max():.5f}]")
+    st = op.lanczos_stats()
+    args.lanczos_stats = st      # carried to the JSON line (finish)
+    log("low modes: where the time went [s]: " + ", ".join(f"{n} {v:.2f}" for n, v in st["seconds"].items())
+        + f"; {st['restarts']} restart cycles, {st['filter_applies']} filter applications, Krylov dimension {st['subspace']}")
     if not ok:
         raise RuntimeError(f"Lanczos did not reach 1e-8 (max residual {res.max():.2e})")
     if path:
@@ -627,7 +631,7 @@ def finish(args, cfg, order, k, V_sites, world, ms, value, launches, tim, e2e, h
                    "dslash_variant": variant_used, "layout": args.layout,
                    "l2": "inputs larger than L2 (gauge 510 MB + 17 GB of low modes stream every step)",
                    "low_modes": f"GPU Lanczos, max residual {resid:.1e}, {lanczos_s:.0f} s (untimed setup)" if k else "none"},
-        "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu, "cg_time_to_solution": cg, "deflated_cg": deflation, "batched": batched, "recon12": recon12,
+        "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu, "lanczos": getattr(args, "lanczos_stats", None), "cg_time_to_solution": cg, "deflated_cg": deflation, "batched": batched, "recon12": recon12,
         "paper_context": "paper: ~30 CPU cores per GPU on unnamed 6 GB GPUs vs Cray XT-5 (PAPER.md:9) - context only",
     }
     print(json.dumps(line), flush=True)

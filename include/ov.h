@@ -242,9 +242,13 @@ int ov_multishift_cg(ov_ctx* ctx, const double* masses_host, int nmass, const vo
                      int maxiter, int* iters_out, double* relres_out);
 int ov_lanczos_lowmodes(ov_ctx* ctx, int k, double tol, int max_restarts, int cheb_order, int subspace,
                         void* V_out_dev, double* lambda_out_host, double* resid_out_host);
-/* statistics of the last ov_lanczos_lowmodes call: out_host[6] = { restart cycles, filter applications (each 2*cheb_order
- * Wilson launches), kernel launches in the call, final lower edge a of the filter window [a,1] of Q^2 (modes with
- * lambda^2 < a are amplified), times the window had to be widened (completeness guard), Krylov dimension m }.  */
+/* statistics of the last ov_lanczos_lowmodes / ov_lanczos_dov_lowmodes call: out_host[12] = { restart cycles, filter
+ * applications (each 2*cheb_order Wilson launches), kernel launches in the call, final lower edge a of the filter window
+ * [a,1] of Q^2 (modes with lambda^2 < a are amplified), times the window had to be widened (completeness guard), Krylov
+ * dimension m, and where the time went, in seconds: [6] the host eigensolver of the projected matrices (device idle),
+ * [7] filter applications, [8] orthogonalisation (two Gram-Schmidt passes + normalisation per step), [9] in-place
+ * rotations of the basis, [10] Rayleigh-Ritz in Q and residual checks (CUDA events on the context's stream), [11] wall
+ * clock of the whole call (the remainder is allocation, the first-guess Lanczos steps and host bookkeeping) }.   */
 int ov_lanczos_stats(const ov_ctx* ctx, double* out_host);
 
 /* ---- low modes of the overlap operator and deflation ("we use deflation to help speed up
@@ -285,9 +289,10 @@ int ov_lanczos_dov_lowmodes(ov_ctx* ctx, int chirality, int k, double tol, int m
                             int subspace, void* W_out_dev, double* mu_out_host, double* resid_out_host);
 int ov_set_deflation(ov_ctx* ctx, const void* W_dev, const double* mu_host, int k);
 
-/* ---- host-logic test hook (no device work): eigen-decomposition of a dense n x n Hermitian matrix by the
- * cyclic complex Jacobi routine the Lanczos driver uses.  A_host: row-major (re,im) pairs; w_out: n ascending
- * eigenvalues; Z_out: row-major (re,im), eigenvectors as columns.                                            */
+/* ---- host-logic test hook (no device work): eigen-decomposition of a dense n x n Hermitian matrix by the routine the
+ * Lanczos driver uses once per restart cycle (Householder tridiagonalisation + implicit-shift QR, on one host core).
+ * A_host: row-major (re,im) pairs, only the lower triangle is read; w_out: n ascending eigenvalues; Z_out: row-major
+ * (re,im), eigenvectors as columns.  OV_ENOCONV if the QR iteration does not converge.                          */
 int ov_host_eigh(int n, const double* A_host, double* w_out, double* Z_out);
 
 #ifdef __cplusplus

@@ -382,7 +382,9 @@ class Overlap:
 
     def lanczos_stats(self):
         """ov_lanczos_stats: counters of the last lanczos_lowmodes call."""
-        out = (ctypes.c_double * 6)()
+        out = (ctypes.c_double * 12)()
         self._check(self.lib.ov_lanczos_stats(self._ctx, out))
         return dict(restarts=int(out[0]), filter_applies=int(out[1]), launches=int(out[2]), edge=out[3],
-                    widenings=int(out[4]), subspace=int(out[5]))
+                    widenings=int(out[4]), subspace=int(out[5]),
+                    seconds=dict(host_eigh=out[6], filter=out[7], orthogonalisation=out[8], rotation=out[9],
+                                 rayleigh_ritz=out[10], total=out[11]))

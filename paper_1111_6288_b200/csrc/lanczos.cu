@@ -12,6 +12,7 @@
 // k = 200 on 32^3x64 (80.5 GB of eigenvectors) runs in 180 GB with a Krylov space of ~1.5 k instead of needing a second
 // copy of the basis (the paper's 2.5 l subspace, would be 201 GB there).
 #include <algorithm>
+#include <chrono>
 #include <cmath>
 #include <functional>
 #include <numeric>
@@ -139,6 +140,40 @@ static int rotate(ov_ctx* ctx, const Basis& W, int m, const std::vector<double2>
     return launch_rotate_inplace(ctx, W.a, W.na, W.b, W.n, m, ncol, d_St);
 }
 
+// Where the time of a run goes (ov_lanczos_stats): CUDA events on the context's stream mark the start of each device
+// phase; flush() synchronises, adds the interval between consecutive marks to the phase of the earlier one and recycles the
+// events.  It is called where the driver synchronises anyway (before the host eigensolver, at the end of a run).
+struct PhaseClock {
+    enum { kFilter = 0, kOrtho = 1, kRotate = 2, kRitz = 3, kPhases = 4 };
+    cudaStream_t stream;
+    std::vector<cudaEvent_t> pool;
+    std::vector<int> phase;
+    size_t used = 0;
+    double ms[kPhases] = {0, 0, 0, 0};
+    explicit PhaseClock(cudaStream_t st) : stream(st) {}
+    ~PhaseClock() { for (auto e : pool) cudaEventDestroy(e); }
+    void mark(int ph) {   // ph = -1: end of the timed stretch
+        if (used == pool.size()) {
+            cudaEvent_t e;
+            if (cudaEventCreate(&e) != cudaSuccess) return;
+            pool.push_back(e);
+            phase.push_back(-1);
+        }
+        phase[used] = ph;
+        cudaEventRecord(pool[used++], stream);
+    }
+    void flush() {
+        if (used == 0) return;
+        mark(-1);
+        cudaStreamSynchronize(stream);
+        for (size_t i = 0; i + 1 < used; i++) {
+            float t = 0.f;
+            if (phase[i] >= 0 && cudaEventElapsedTime(&t, pool[i], pool[i + 1]) == cudaSuccess) ms[phase[i]] += t;
+        }
+        used = 0;
+    }
+};
+
 static double inverse_filter(const Filter& f, double theta_abs) {
     // x < a with |T_d(z(x))| = theta_abs  ->  |z| = cosh(acosh(theta)/d)
     if (theta_abs <= 1.0) return f.a;
@@ -152,7 +187,7 @@ using namespace ov;
 
 extern "C" int ov_lanczos_stats(const ov_ctx* ctx, double* out_host) {
     if (!ctx || !out_host) return OV_EINVAL;
-    for (int i = 0; i < 6; i++) out_host[i] = ctx->lanczos_stats[i];
+    for (size_t i = 0; i < ctx->lanczos_stats.size(); i++) out_host[i] = ctx->lanczos_stats[i];
     return OV_OK;
 }
 
@@ -222,7 +257,7 @@ static int lanczos_driver(ov_ctx* ctx, const LanczosOp& op, int k, double tol, i
             OV_TRY(normalise(u, &nrm));
             if (j + 1 < m0) { T[(size_t)j * m0 + j + 1].x = nrm; T[(size_t)(j + 1) * m0 + j].x = nrm; }
         }
-        host_eigh(m0, T, th, S);
+        if (!host_eigh(m0, T, th, S)) return fail(ctx, OV_ENOCONV, "dense eigensolver: QR iteration did not converge");
         theta_min = std::max(th[0], 1e-12);
     }
     Filter f{cheb_order, op.edge0(theta_min), op.bmax};
@@ -237,13 +272,41 @@ static int lanczos_driver(ov_ctx* ctx, const LanczosOp& op, int k, double tol, i
     const long long launches0 = ctx->launches;
     ctx->lanczos_stats = {};
     int rc_final = OV_ENOCONV;
+    PhaseClock clk(ctx->stream);
+    double eigh_s = 0.0;
+    const auto wall0 = std::chrono::steady_clock::now();
+    auto seconds_since = [](std::chrono::steady_clock::time_point t0) {
+        return std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count();
+    };
+    auto timed_eigh = [&](int nn, std::vector<double2>& A, std::vector<double>& w, std::vector<double2>& Z) {
+        clk.flush();                                    // the device is idle from here until the decomposition is back
+        const auto t0 = std::chrono::steady_clock::now();
+        const bool ok = host_eigh(nn, A, w, Z);
+        eigh_s += seconds_since(t0);
+        return ok;
+    };
+    auto write_times = [&]() {
+        clk.flush();
+        ctx->lanczos_stats[6] = eigh_s;
+        ctx->lanczos_stats[7] = 1e-3 * clk.ms[PhaseClock::kFilter];
+        ctx->lanczos_stats[8] = 1e-3 * clk.ms[PhaseClock::kOrtho];
+        ctx->lanczos_stats[9] = 1e-3 * clk.ms[PhaseClock::kRotate];
+        ctx->lanczos_stats[10] = 1e-3 * clk.ms[PhaseClock::kRitz];
+        ctx->lanczos_stats[11] = seconds_since(wall0);
+    };
     // start vector: W[0] stays (normalised random)
     for (int restart = 0; restart < max_restarts; restart++) {
-        ctx->lanczos_stats = {(double)(restart + 1), (double)filter_applies, 0.0, f.a, (double)widenings, (double)m};
+        ctx->lanczos_stats[0] = (double)(restart + 1);
+        ctx->lanczos_stats[1] = (double)filter_applies;
+        ctx->lanczos_stats[3] = f.a;
+        ctx->lanczos_stats[4] = (double)widenings;
+        ctx->lanczos_stats[5] = (double)m;
         for (int j = l; j < m; j++) {
             double2* u = W.vec(j + 1);
+            clk.mark(PhaseClock::kFilter);
             OV_TRY(op.filter(f, W.vec(j), u, t1, tq));
             filter_applies++;
+            clk.mark(PhaseClock::kOrtho);
             OV_TRY(cgs_pass(ctx, W, j + 1, u, d_C, c));
             double alpha = c[j].x;
             OV_TRY(cgs_pass(ctx, W, j + 1, u, d_C, c));
@@ -254,7 +317,7 @@ static int lanczos_driver(ov_ctx* ctx, const LanczosOp& op, int k, double tol, i
         }
         const double beta_last = nrm;
         std::vector<double2> Tc = T;
-        host_eigh(m, Tc, th, S);
+        if (!timed_eigh(m, Tc, th, S)) return fail(ctx, OV_ENOCONV, "dense eigensolver: QR iteration did not converge");
         std::vector<int> idx(m);
         std::iota(idx.begin(), idx.end(), 0);
         std::sort(idx.begin(), idx.end(), [&](int a, int b2) { return std::fabs(th[a]) > std::fabs(th[b2]); });
@@ -266,7 +329,9 @@ static int lanczos_driver(ov_ctx* ctx, const LanczosOp& op, int k, double tol, i
             if (res > tolB * std::fabs(th[kept[i]])) { conv = false; break; }
         }
         // Ritz vectors of the kept set, in place: W[0..keep) <- W[0..m) S[:, kept]
+        clk.mark(PhaseClock::kRotate);
         OV_TRY(rotate(ctx, W, m, S, m, kept, d_St));
+        clk.mark(-1);
         // projected matrix in the rotated basis: diag(theta) + the coupling to the residual vector W[m]
         std::vector<double2> Tk((size_t)keep * keep, make_double2(0, 0)), zk(keep);
         for (int i = 0; i < keep; i++) {
@@ -308,6 +373,7 @@ static int lanczos_driver(ov_ctx* ctx, const LanczosOp& op, int k, double tol, i
             // Rayleigh-Ritz in R on span(W[0..keep)): M = Y^+ R Y
             std::vector<double2> M((size_t)keep * keep), SM;
             std::vector<double> mu;
+            clk.mark(PhaseClock::kRitz);
             for (int j = 0; j < keep; j++) {
                 OV_TRY(op.rr(W.vec(j), tq, t2));
                 OV_TRY(basis_dots(ctx, W, keep, tq));
@@ -322,13 +388,15 @@ static int lanczos_driver(ov_ctx* ctx, const LanczosOp& op, int k, double tol, i
                     M[(size_t)i * keep + j] = h;
                     M[(size_t)j * keep + i] = make_double2(h.x, -h.y);
                 }
-            host_eigh(keep, M, mu, SM);
+            if (!timed_eigh(keep, M, mu, SM)) return fail(ctx, OV_ENOCONV, "dense eigensolver: QR iteration did not converge");
             std::vector<int> order(keep);
             std::iota(order.begin(), order.end(), 0);
             std::sort(order.begin(), order.end(), [&](int a, int b2) { return std::fabs(mu[a]) < std::fabs(mu[b2]); });
             // rotate the whole kept block by the unitary R = SM[:, order], in place: the wanted k eigenvectors of Q land in
             // W[0..k) = the caller's buffer, and W[0..keep) stays an orthonormal basis of the same space
+            clk.mark(PhaseClock::kRotate);
             OV_TRY(rotate(ctx, W, keep, SM, keep, order, d_St));
+            clk.mark(PhaseClock::kRitz);
             double worst = 0.0;
             for (int i = 0; i < k; i++) {
                 double2* v = W.vec(i);
@@ -342,6 +410,7 @@ static int lanczos_driver(ov_ctx* ctx, const LanczosOp& op, int k, double tol, i
                 resid_out_host[i] = std::sqrt(r2);
                 worst = std::max(worst, resid_out_host[i]);
             }
+            clk.mark(-1);
             if (worst <= tol) { rc_final = OV_OK; break; }
             tolB *= 0.1;  // not there yet: ask more of the Krylov space and go on, in the rotated basis
             std::vector<double2> R((size_t)keep * keep), tmp((size_t)keep * keep), z2(keep);
@@ -383,6 +452,7 @@ static int lanczos_driver(ov_ctx* ctx, const LanczosOp& op, int k, double tol, i
     ctx->lanczos_stats[2] = (double)(ctx->launches - launches0);
     ctx->lanczos_stats[3] = f.a;
     ctx->lanczos_stats[4] = (double)widenings;
+    write_times();
     OV_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     if (rc_final != OV_OK) return fail(ctx, OV_ENOCONV, "lanczos: residual above tol after %d restarts", max_restarts);
     return OV_OK;

@@ -85,7 +85,8 @@ struct ov_ctx {
     void* tma_state = nullptr; // tensor maps and schedule of the TMA-staged kernel (wilson_tma.cu)
     bool tma_ok = true;        // false: tma_probe failed at ov_create_ex, the context never picks the TMA-staged kernel
     std::vector<int> cg_orders;  // order used at each iteration of the last adaptive CG (negative: fp32 sweep)
-    std::array<double, 6> lanczos_stats{};  // last ov_lanczos_lowmodes: restarts, filter applies, launches, edge a, widenings, m
+    std::array<double, 12> lanczos_stats{};  // last eigensolver run: restarts, filter applies, launches, edge a, widenings, m,
+                                             // then seconds: host eigensolver, filter, orthogonalisation, rotations, Rayleigh-Ritz, total
     int cg_adaptive = 0;  // ov_set_cg_adaptive: 0 off, 1 reduced orders, 2 reduced orders + fp32 sweeps
     int cg_operator = 0;  // ov_set_cg_operator: 0 gamma5 D gamma5 D, 1 chirally symmetric form 2 + gamma5 S + S gamma5
     int cg_chirality = 0; // last solve in the symmetric form: chirality of the source the solver detected (0 = none)
@@ -178,9 +179,9 @@ void tma_state_free(ov_ctx* ctx);
 // batched: nrhs consecutive ABI spinors (stride 12 V) in in/out and in every epilogue operand
 int launch_wilson_batch(ov_ctx* ctx, const double2* in, double2* out, const Epilogue& ep, int nrhs);
 int launch_wilson_gather_f32(ov_ctx* ctx, const float2* in, float2* out, const EpilogueF& ep);  // needs ctx->gauge_f
-// host-side dense Hermitian eigensolver (cyclic complex Jacobi): A (n x n, row-major complex, destroyed),
-// w ascending, Z row-major with eigenvectors as COLUMNS
-void host_eigh(int n, std::vector<double2>& A, std::vector<double>& w, std::vector<double2>& Z);
+// host-side dense Hermitian eigensolver (Householder tridiagonalisation + implicit-shift QR): A (n x n, row-major complex,
+// destroyed), w ascending, Z row-major with eigenvectors as COLUMNS; false = no convergence
+bool host_eigh(int n, std::vector<double2>& A, std::vector<double>& w, std::vector<double2>& Z);
 
 // BLAS-1 on ABI spinors (n = 12 V complex)
 int launch_axpy(ov_ctx* ctx, double2 a, const double2* x, double2* y);                     // y += a x

@@ -39,7 +39,7 @@ def test_chebyshev_coeffs_match_oracle_generator(lib):
 
 def test_host_eigh_against_numpy(lib):
     rng = np.random.default_rng(0)
-    for n in (1, 2, 5, 40, 130):
+    for n in (1, 2, 3, 5, 40, 130, 216):
         A = rng.standard_normal((n, n)) + 1j * rng.standard_normal((n, n))
         A = A + A.conj().T
         w, Z = ovp.host_eigh(A)
@@ -56,6 +56,21 @@ def test_host_eigh_against_numpy(lib):
     w, Z = ovp.host_eigh(T)
     assert np.max(np.abs(w - np.linalg.eigvalsh(T))) < 1e-12
     assert np.max(np.abs(T @ Z - Z * w)) < 1e-12
+    # degenerate spectra (no rotation needed / all equal / repeated) and the size of configs[4]'s Krylov space, which must
+    # not stall the GPU for seconds per restart cycle any more (the Jacobi sweeps of rounds 1-2 took 8.9 s here)
+    for A in (np.eye(7), np.zeros((6, 6)), np.diag([3.0, 1.0, 2.0, 2.0, -1.0])):
+        w, Z = ovp.host_eigh(A.astype(np.complex128))
+        assert np.array_equal(w, np.sort(np.diag(A))) and np.max(np.abs(A @ Z - Z * w)) == 0.0
+    import time
+    n = 416
+    A = rng.standard_normal((n, n)) + 1j * rng.standard_normal((n, n))
+    A = A + A.conj().T
+    t0 = time.perf_counter()
+    w, Z = ovp.host_eigh(A)
+    assert time.perf_counter() - t0 < 3.0
+    assert np.max(np.abs(w - np.linalg.eigvalsh(A))) < 1e-11 * np.abs(w).max()
+    assert np.max(np.abs(Z.conj().T @ Z - np.eye(n))) < 1e-12
+    assert np.max(np.abs(A @ Z - Z * w)) < 1e-10 * np.abs(w).max()
 
 
 def test_no_cpu_fallback(lib):
