@@ -89,7 +89,7 @@ def check_modes_with_oracle(cfg, U, Vh, lam):
     return worst_res
 
 
-def run_dov_config(ovp, cfg, nsrc_checked, parity_log, lanczos_order=100):
+def run_dov_config(ovp, cfg, nsrc_checked, parity_log, lanczos_order=100, recon12=False):
     U = wl.su3_links(cfg.dims, cfg.spread, wl.gauge_seed(cfg.index))
     op = ovp.Overlap(cfg.dims, cfg.kappa, U)
     coef = ovp.chebyshev_coeffs(cfg.order, cfg.eps)
@@ -107,12 +107,29 @@ def run_dov_config(ovp, cfg, nsrc_checked, parity_log, lanczos_order=100):
         x = wl.gaussian_source(cfg.dims, wl.source_seed(cfg.index, j))
         got = host(op, op.apply_dov(0.0, dev(op, x)))
         ref = oracle.dov(cfg.dims, cfg.kappa, U, coef, cfg.eps, cfg.norm, Vh, lam, 0.0, x)
+        if j == 0:
+            ref0 = ref
         errs.append(rel(got, ref))
         parity_log(f"configs[{cfg.index}] {cfg.name} D_ov rel-L2 (n={cfg.order}, k={cfg.k}, source {j})", errs[-1], TOL_DOV)
         assert errs[-1] <= TOL_DOV
-    # the host-buffer entry point (what bench.py's e2e times) gives the same answer as the device entry point
-    x = wl.gaussian_source(cfg.dims, wl.source_seed(cfg.index, 0))
-    assert rel(op.apply_dov_host(0.0, x), host(op, op.apply_dov(0.0, dev(op, x)))) <= 1e-14
+    # the host-buffer entry point (what bench.py's e2e times) gives the same answer as the device entry point: one source
+    # (single-buffered staging) and three (double-buffered copies overlapping the operator), with the small space set
+    xs = np.stack([wl.gaussian_source(cfg.dims, wl.source_seed(cfg.index, j)) for j in range(3)])
+    want = [host(op, op.apply_dov(0.0, dev(op, xs[j]))) for j in range(3)]
+    assert rel(op.apply_dov_host(0.0, xs[0]), want[0]) <= 1e-14
+    got3 = op.apply_dov_host(0.0, xs)
+    for j in range(3):
+        assert rel(got3[j], want[j]) <= 1e-14
+    if recon12:
+        # the same apply with 12-real links (what bench.py reports as `recon12`), against the oracle reference of source 0
+        x0 = wl.gaussian_source(cfg.dims, wl.source_seed(cfg.index, 0))
+        op12 = ovp.Overlap(cfg.dims, cfg.kappa, U, recon=12)
+        op12.set_polynomial(coef, cfg.eps, cfg.norm)
+        op12.set_smallspace(V, lam)
+        e12 = rel(host(op12, op12.apply_dov(0.0, dev(op12, x0))), ref0)
+        parity_log(f"configs[{cfg.index}] {cfg.name} recon-12 D_ov rel-L2 (n={cfg.order}, k={cfg.k}, source 0)", e12, TOL_DOV)
+        assert e12 <= TOL_DOV
+        op12.close()
     return errs
 
 
@@ -124,21 +141,26 @@ def test_config3_headline_hw_all_sources_and_dov(ovp, parity_log):
     cfg = wl.CONFIGS[3]
     U = wl.su3_links(cfg.dims, cfg.spread, wl.gauge_seed(cfg.index))
     op = ovp.Overlap(cfg.dims, cfg.kappa, U)
-    worst = 0.0
+    op12 = ovp.Overlap(cfg.dims, cfg.kappa, U, recon=12)     # 12-real links: bench.py times them at this size
+    worst = worst12 = 0.0
     for j in range(cfg.nsrc):
         x = wl.gaussian_source(cfg.dims, wl.source_seed(cfg.index, j))
         ref = oracle.hw(cfg.dims, cfg.kappa, U, x)
         d = dev(op, x)
         worst = max(worst, rel(host(op, op.apply_hw(d)), ref))
-        assert worst <= TOL_HW
+        worst12 = max(worst12, rel(host(op12, op12.apply_hw(d)), ref))
+        assert worst <= TOL_HW and worst12 <= TOL_HW
         if j == 0:
             e32 = rel(host(op, op.apply_hw_f32(d)), ref)
             parity_log("configs[3] 24^3x64 fp32 H_w rel-L2", e32, TOL_HW_F32)
             assert e32 <= TOL_HW_F32
     parity_log("configs[3] 24^3x64 fp64 H_w rel-L2, worst of 8 sources", worst, TOL_HW)
-    del op
+    parity_log("configs[3] 24^3x64 fp64 H_w with 12-real links rel-L2, worst of 8 sources", worst12, TOL_HW)
+    assert op12.dslash_variant == op.dslash_variant == 2
+    op12.close()
+    del op, op12
     torch.cuda.empty_cache()
-    run_dov_config(ovp, cfg, 1, parity_log)
+    run_dov_config(ovp, cfg, 1, parity_log, recon12=True)
 
 
 def test_plane_wave_closed_form_at_24x64(ovp):
@@ -362,6 +384,9 @@ def test_deflated_cg_16x32_hard_workload(ovp, parity_log):
     print(f"  multi-mass CG, 6 masses, tol 1e-8: plain {it_plain} iterations {t_plain:.1f} s, deflated (2 x {k} modes) "
           f"{it_defl} iterations {t_defl:.1f} s; true residuals plain {res_plain.max():.2e}, deflated {res_defl.max():.2e}")
     assert ok1 and ok2
+    # the solver stops when the RECURSIVE residual of the slowest system is <= tol |b|; res_* are the TRUE residuals it
+    # recomputes with the operator afterwards.  Over ~300 (plain) iterations the recurrence drifts from the true residual
+    # by rounding, so the gate is tol plus 20 % for that drift (the observed values are printed above), not tol itself
     assert np.all(res_plain <= 1.2e-8) and np.all(res_defl <= 1.2e-8)
     parity_log(f"16^3x32 hard workload: CG iterations plain / deflated = {it_plain} / {it_defl} (gate: 2 deflated <= plain)",
                2.0 * it_defl / it_plain, 1.0)
@@ -377,6 +402,10 @@ def test_deflated_cg_16x32_hard_workload(ovp, parity_log):
         Ax = dfl.normal_op(lambda u: oracle.dov(*args, 0.0, u), xh)
     sg = sigma_of_mass(cfg.masses[0])
     e = float(np.linalg.norm((b - Ax - sg * xh).ravel()) / np.linalg.norm(b.ravel()))
+    # gate: the library's own true residual (<= 1.2e-8 above) plus what the two implementations of A may differ by on this
+    # x: |A_gpu x - A_oracle x| <= 2 * 1e-10 |x| (two D_ov applies at the 1e-10 parity gate) with |x| / |b| up to
+    # 1/(mu_0 + sigma_0) ~ 4e4, i.e. up to 8e-6 in the worst case allowed by the parity gate, ~1e-15 * 4e4 in practice;
+    # 2e-8 leaves 0.8e-8 for it
     parity_log("16^3x32 deflated solution, lightest mass: true residual with the ORACLE's D_ov", e, 2e-8)
     assert e <= 2e-8
 

@@ -353,6 +353,37 @@ def test_batched_apply_matches_single_and_oracle(ovp, cfg0, with_small):
     assert rel(got_d[6], ref) <= TOL_DOV
 
 
+def test_batched_gather_sweep_vs_oracle_on_many_blocks(ovp, parity_log):
+    """The batched Clenshaw sweep of the GATHER kernel (two right-hand sides per thread block sharing the link loads, fused
+    axpy operands with a right-hand-side stride) meets the oracle on a lattice the TMA-staged kernel does not take
+    (X = 6) and that spans many thread blocks (2880 sites; 4^4, the other non-TMA test lattice, is 4 blocks), with a
+    small space: nrhs = 5 = one batch of 4 and a single.  The low modes come from the library's Lanczos and are
+    re-verified with the oracle's H_w before the oracle uses them."""
+    dims, spread, n, se, k = (6, 10, 6, 8), 0.5, 24, 0.05, 6
+    U = wl.su3_links(dims, spread, 31)
+    op = make(ovp, dims, U)
+    assert op.dslash_variant == 1 and op.spinor_layout == 1
+    coef = ovp.chebyshev_coeffs(n, se * se)
+    op.set_polynomial(coef, se * se, NORM)
+    V, lam, res, ok = op.lanczos_lowmodes(k, tol=1e-10, max_restarts=80, cheb_order=40)
+    assert ok and np.all(res <= 1e-10)
+    Vh = to_host(op, V)
+    for i in range(k):
+        assert np.linalg.norm((oracle.hw(dims, KAPPA, U, Vh[i]) / NORM - lam[i] * Vh[i]).ravel()) <= 1e-9
+    op.set_smallspace(V, lam)
+    xs = np.stack([wl.gaussian_source(dims, 80 + j) for j in range(5)])
+    got_d, got_s = to_host(op, op.apply_dov(0.07, to_dev(op, xs))), to_host(op, op.apply_sign(to_dev(op, xs)))
+    for j in (0, 3, 4):                                       # first and last of the batch of 4, and the single
+        ref = oracle.dov(dims, KAPPA, U, coef, se * se, NORM, Vh, lam, 0.07, xs[j])
+        e = rel(got_d[j], ref)
+        parity_log(f"6x10x6x8 batched gather sweep (nrhs=5, k={k}, n={n}): D_ov rel-L2, rhs {j}", e, TOL_DOV)
+        assert e <= TOL_DOV
+    ref = oracle.sign(dims, KAPPA, U, coef, se * se, NORM, Vh, lam, xs[2])
+    assert rel(got_s[2], ref) <= TOL_DOV
+    for j in range(5):                                        # and every rhs equals its own nrhs = 1 call bit for bit
+        assert np.array_equal(got_d[j], to_host(op, op.apply_dov(0.07, to_dev(op, xs[j]))))
+
+
 @pytest.mark.parametrize("k", [401, 801])
 def test_batched_projector_with_many_modes(ovp, cfg0, k):
     """The batched V^+ x keeps 128 B of shared memory per (mode, rhs): groups of 4 fit up to k = 400, groups of 2 up to 800.
